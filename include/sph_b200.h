@@ -1,0 +1,184 @@
+/* sph_b200.h - C ABI of libsph_b200.so: the data-parallel hot path of the SPH time step of
+ * arXiv 1210.1017 (Valdez-Balderas, Dominguez, Rogers, Crespo), hand-written for NVIDIA
+ * B200 (sm_100a).  Citations "Lnnn" are line numbers of the paper text PAPER.md.
+ *
+ * The path (one call each, or all of them through sph_step):
+ *   sph_sort_and_cells  L138-140  cell label per particle, radix sort of the particles by
+ *                                 (cell, id), re-ordering of all state arrays, index of the
+ *                                 first particle of every cell; the same pass tags edge
+ *                                 ("halo") and migrating particles (L240, L264)
+ *   sph_build_halos     L192, L198-219, L224-228, L240-264  halo of every logical x-slab
+ *                                 sub-domain (= edge of its neighbours, width 2h) gathered
+ *                                 into halo buffers; migrating particles compacted
+ *   sph_interact        L101-112, L116, L142-146  right-hand sides of Eqs. (7) and (9)
+ *   sph_step            L126-150  all of the above, then the Verlet update (L150)
+ *
+ * Conventions
+ *   - Every pointer argument says HOST or DEVICE.  The library never allocates device memory:
+ *     the caller passes one DEVICE workspace of sph_workspace_bytes() bytes (256-byte
+ *     aligned) that must outlive the context, and a CUDA stream (cudaStream_t as void*,
+ *     NULL = legacy default stream).  Inputs are copied at sph_init / sph_set_state; no
+ *     caller memory is referenced afterwards.
+ *   - Calls only ENQUEUE work on the stream and return, except sph_download, sph_status,
+ *     sph_profile_read and sph_init/sph_set_state with HOST inputs, which synchronise it.
+ *   - Return value: SPH_OK (0) or a negative SPH_ERR_* code; no exceptions, no abort, no
+ *     CPU fallback.  sph_strerror() names a code.
+ *   - Particle k of the input has id k.  n < 2^28; number of grid cells <= 2^28.
+ *   - Precision: fp32 state and arithmetic (the paper does not state its precision, L35).
+ */
+#ifndef SPH_B200_H
+#define SPH_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SPH_MAX_SLABS 16
+
+enum {
+    SPH_OK = 0,
+    SPH_ERR_ARG = -1,             /* NULL / out-of-range argument */
+    SPH_ERR_WORKSPACE = -2,       /* workspace NULL, misaligned or too small */
+    SPH_ERR_GRID_TOO_LARGE = -3,  /* more than 2^28 cells, or n >= 2^28 */
+    SPH_ERR_SLABS = -4,           /* planes not 0 = p0 < p1 < ... < pS = ncx, a slab thinner
+                                     than 2 cell planes (S > 1), or S > max_slabs */
+    SPH_ERR_CUDA = -5,            /* a CUDA runtime call failed (sticky) */
+    SPH_ERR_NONFINITE = -6,       /* a non-finite position/velocity/density was seen on the
+                                     device (sticky flag, reported by sph_status) */
+    SPH_ERR_ORDER = -7            /* call order violated (e.g. sph_interact before a sort) */
+};
+
+typedef struct sph_ctx sph_ctx;   /* opaque */
+
+/* Physical and grid parameters (all plain values, copied at sph_init). */
+typedef struct {
+    float dp;                     /* initial particle spacing (used only to size work items) */
+    float h;                      /* smoothing length; kernel support and cell side are 2h (L81, L140) */
+    float rho0, c0, alpha;        /* Tait reference density and sound speed, viscosity alpha (L112) */
+    int   gamma;                  /* Tait exponent, 1..15 (paper: 7) */
+    float g[3];                   /* gravity, added to fluid particles (Eq. 9) */
+    float mass_fluid, mass_bound; /* particle masses by type */
+    float dom_min[3], dom_max[3]; /* cell grid: nc = ceil((max-min)/(2h)) per axis; cell indices
+                                     are clamped to the grid (particles are never dropped) */
+    int   verlet_ns;              /* every verlet_ns-th step (and step 0) is the one-sided
+                                     corrective step; <= 0: step 0 only */
+    int   kernel;                 /* 0 = Wendland C2 (hot path), 1 = cubic spline (paper L81) */
+} sph_params;
+
+/* Input particles, id order.  Arrays are HOST pointers (on_device = 0) or DEVICE pointers
+ * (on_device = 1), owned by the caller, read during the call only. */
+typedef struct {
+    uint64_t n;
+    const float *pos;             /* n*3 (x,y,z interleaved) */
+    const float *vel;             /* n*3 */
+    const float *rho;             /* n   */
+    const uint8_t *type;          /* n, 0 = fluid, 1 = dynamic boundary particle (L116); NULL = all fluid */
+    const uint8_t *prev_slab;     /* n, previous owner sub-domain used by the FIRST sort after
+                                     this call to label migrants (L264); NULL = no migrants */
+    int on_device;
+} sph_particles;
+
+/* Borrowed DEVICE pointers into the workspace; valid until the next sph_* call that
+ * changes state on this context.  Arrays are in sorted (cell, id) order after a sort. */
+typedef struct {
+    uint64_t n;
+    int32_t  nc[3];               /* cells per axis */
+    uint32_t ncells;
+    int32_t  cell_bits;           /* bits of the keyword that are sorted */
+    int32_t  n_slabs;
+    uint64_t step_index;          /* number of completed sph_step calls */
+    const float *pos4;            /* n float4: x, y, z, p/rho^2 */
+    const float *velrho4;         /* n float4: vx, vy, vz, rho */
+    const float *velrhoM1_4;      /* n float4: Verlet n-1 velocity and density */
+    const float *acc4;            /* n float4: ax, ay, az, d rho/dt (after sph_interact) */
+    const uint32_t *idt;          /* n: id in bits 0..27, type in bit 31 */
+    const uint32_t *keyword;      /* n: cell in bits 0..27, edge label bits 28..29 (L240: 1 left,
+                                     2 right), migration label bits 30..31 (L264: 1 left, 2 right) */
+    const uint32_t *cell_begin;   /* ncells+1: index of the first particle of each cell
+                                     (lower bound; cell_end[c] == cell_begin[c+1]) */
+    const uint32_t *slab_begin;   /* n_slabs+1: first particle of each slab; owned[s] = diff */
+    const uint32_t *halo_offset;  /* 2*n_slabs+1: halo 2s = left halo of slab s, 2s+1 = right
+                                     halo; entries [halo_offset[k], halo_offset[k+1]) of: */
+    const float *halo_pos4;
+    const float *halo_velrho4;
+    const uint32_t *halo_idt;
+    const uint32_t *mig_total;    /* 1: number of migrant records */
+    const uint32_t *migrants;     /* mig_total uint4 records (id, sortedIndex, prevSlab, slab),
+                                     in sorted order */
+    const uint32_t *mig_count;    /* n_slabs*2: particles that left slab s to the left / right */
+} sph_view;
+
+/* Stage timers (sph_profile_*): indices into the ms[] array. */
+enum {
+    SPH_T_KEYS = 0, SPH_T_SORT, SPH_T_GATHER, SPH_T_CELLS, SPH_T_HALO, SPH_T_MIGRATE,
+    SPH_T_INTERACT, SPH_T_VERLET, SPH_T_COUNT
+};
+
+/* Options for sph_set_option. */
+enum {
+    SPH_OPT_INTERACT_VARIANT = 0  /* 0 = smem-staged production kernel, 1 = simple
+                                     one-thread-per-particle kernel (cross-check) */
+};
+
+/* Bytes of DEVICE workspace needed for n_max particles and max_slabs sub-domains with the
+ * grid of *p.  Returns 0 on bad arguments or a grid above 2^28 cells. */
+size_t sph_workspace_bytes(const sph_params *p, uint64_t n_max, int max_slabs);
+
+/* Create a context.  workspace: DEVICE, >= sph_workspace_bytes(p, part->n, max_slabs) bytes.
+ * Copies the particles in (id order), computes p/rho^2, sets step_index = 0, one slab. */
+int sph_init(sph_ctx **out, const sph_params *p, const sph_particles *part, int max_slabs,
+             void *workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* Replace the whole particle state (same n) and reset step_index; HOST or DEVICE inputs. */
+int sph_set_state(sph_ctx *ctx, const sph_particles *part);
+
+/* Set the logical sub-domains: planes HOST int32[n_slabs+1], planes[0] = 0 < ... <
+ * planes[n_slabs] = nc[0] (cell-plane indices along x, reading A14/A17).  Takes effect at the
+ * next sort; sph_build_halos(planes) is the usual way to set them. */
+int sph_set_slabs(sph_ctx *ctx, const int32_t *planes, int n_slabs);
+
+/* Snap physical x bounds (HOST float[n_slabs+1]) to cell planes (HOST int32[n_slabs+1] out). */
+int sph_slab_planes_from_x(const sph_ctx *ctx, const float *x_bounds, int n_slabs, int32_t *planes_out);
+
+/* a1-a4: keys+tags, radix sort by (cell, id), payload permutation, cell table, slab ranges. */
+int sph_sort_and_cells(sph_ctx *ctx);
+
+/* a5-a6: halo gather and migrant compaction for the given planes (HOST; NULL = keep the
+ * current ones).  Needs a sort since the last state change.  If the planes differ from the
+ * ones the last sort tagged with, edge labels are recomputed. */
+int sph_build_halos(sph_ctx *ctx, const int32_t *planes, int n_slabs);
+
+/* a7: acc4 = (dv/dt, d rho/dt) of every particle.  Needs the cell table. */
+int sph_interact(sph_ctx *ctx);
+
+/* a1-a8 in order; dt > 0. */
+int sph_step(sph_ctx *ctx, float dt);
+
+int sph_get_view(sph_ctx *ctx, sph_view *out);
+
+/* HOST outputs in ID order, any of them may be NULL: pos n*3, vel n*3, rho n, acc n*3, drho n.
+ * Synchronises the stream. */
+int sph_download(sph_ctx *ctx, float *pos, float *vel, float *rho, float *acc, float *drho);
+
+/* Synchronise the stream; return the sticky error (SPH_OK, SPH_ERR_CUDA, SPH_ERR_NONFINITE). */
+int sph_status(sph_ctx *ctx);
+
+int sph_set_option(sph_ctx *ctx, int option, int value);
+
+/* CUDA-event stage timers on the context's stream.  enable != 0 starts recording an event
+ * pair around every stage of every call; sph_profile_read synchronises, ADDS the elapsed
+ * milliseconds of all recorded pairs to ms[SPH_T_COUNT] and the number of pairs to
+ * launches[SPH_T_COUNT] (HOST arrays, may be NULL), then clears the record. */
+int sph_profile_enable(sph_ctx *ctx, int enable);
+int sph_profile_read(sph_ctx *ctx, float *ms, int *launches);
+
+void sph_destroy(sph_ctx *ctx);
+const char *sph_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPH_B200_H */

@@ -1,0 +1,332 @@
+// a7 - particle interactions ("If particle i is in cell c, the thread will
+// look for neighbours only in cell c and in cells adjacent to c ... compute the interaction
+// between particle i and its neighbours, that is, the sum on the right-hand side of equations
+// (7)-(9)").  Physics: Eq. (7), Eq. (9) L106 (p/rho^2 form, reading A2),
+// artificial viscosity and Tait equation of state L112, dynamic boundary particles L116.
+//
+// Two kernels:
+//  * interact_staged_kernel (production).  A CTA owns a z-run of `zb` cells of one (cx,cy)
+//    column.  With z-fastest keys the candidates of all its targets are 9 contiguous sorted
+//    ranges (one per neighbouring column); they are staged once in shared memory.  Each thread
+//    owns one target particle and works in two phases so that warps stay converged:
+//      filter - stream its 27-cell window from shared memory (broadcast reads), 6 flops + a
+//               compare per candidate, push the smem index of every candidate inside 2h on a
+//               private shared-memory stack;
+//      drain  - whenever a stack in the warp is nearly full (and at the end) all lanes pop one
+//               entry and evaluate the full pair term, so the expensive path runs with (almost)
+//               all lanes active instead of the ~14 % a fused test+interact loop would have.
+//  * interact_simple_kernel (cross-check, SPH_OPT_INTERACT_VARIANT = 1): one thread per
+//    particle walking the cell table with global loads, as the paper describes it.
+//
+// FP32-ALU bound (no tensor cores: this is not a dense contraction).
+#include "sph_internal.cuh"
+
+namespace sph {
+
+// ---- pair term ---------------------------------------------------------------------------------
+// Returns F with grad_i W_ij = F r_ij, for 0 < r2 < 4h^2.
+template <int KERNEL>
+__device__ __forceinline__ float kernel_F(float r2, const PhysC &ph)
+{
+    float rinv = rsqrtf(r2);
+    float r = r2 * rinv;
+    if (KERNEL == 0) {                      // Wendland C2: F = -5 aD (1 - q/2)^3 / h^2
+        float t = fmaf(-ph.inv_h_half, r, 1.0f);
+        return ph.kF * t * t * t;
+    } else {                                // cubic spline, kF = aD / h^2
+        float q = r * (2.0f * ph.inv_h_half);
+        float t = 2.0f - q;
+        float f = q <= 1.0f ? fmaf(2.25f, q, -3.0f) : -0.75f * t * t * rinv * ph.h;
+        return ph.kF * f;
+    }
+}
+
+__device__ __forceinline__ float sound_speed(float rho, const PhysC &ph)
+{
+    float x = rho * ph.inv_rho0;
+    if (ph.gamma == 7) return ph.c0 * x * x * x;
+    return ph.c0 * __powf(x, 0.5f * (float)(ph.gamma - 1));
+}
+
+// Adds the contribution of neighbour j to (ax, ay, az, dr); masses are applied by the caller
+// (mj = 1 in the uniform-mass path).
+template <int KERNEL>
+__device__ __forceinline__ void pair_term(float dx, float dy, float dz, float r2,
+                                          float vxi, float vyi, float vzi, float rhoi, float Pi_, float ci,
+                                          float4 vj, float Pj, float mj, const PhysC &ph,
+                                          float &ax, float &ay, float &az, float &dr)
+{
+    float F = kernel_F<KERNEL>(r2, ph) * mj;
+    float dvx = vxi - vj.x, dvy = vyi - vj.y, dvz = vzi - vj.z;
+    float dot = fmaf(dvz, dz, fmaf(dvy, dy, dvx * dx));
+    dr = fmaf(F, dot, dr);                                            // Eq. (7)
+    float visc = 0.0f;
+    if (dot < 0.0f) {                                                 // L112
+        float cj = sound_speed(vj.w, ph);
+        // Pi = -alpha cbar mu / rhobar = -alpha h (ci+cj) dot / ((r2+eta2)(rhoi+rhoj))
+        visc = -ph.alpha_h * (ci + cj) * dot * __frcp_rn((r2 + ph.eta2) * (rhoi + vj.w));
+    }
+    float coef = -F * (Pi_ + Pj + visc);                              // Eq. (9)
+    ax = fmaf(coef, dx, ax);
+    ay = fmaf(coef, dy, ay);
+    az = fmaf(coef, dz, az);
+}
+
+// ---- simple cross-check kernel -----------------------------------------------------------------
+template <int KERNEL>
+__global__ void __launch_bounds__(128)
+interact_simple_kernel(uint32_t n, const float4 *__restrict__ pos4, const float4 *__restrict__ velrho4,
+                       const uint32_t *__restrict__ idt, const uint32_t *__restrict__ keyword,
+                       const uint32_t *__restrict__ cell_begin, float4 *__restrict__ acc4, GridC g, PhysC ph)
+{
+    uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    float4 pi = pos4[i];
+    float4 vi = velrho4[i];
+    uint32_t cell = keyword[i] & CELL_MASK;
+    int cz = cell % g.nc[2];
+    int cy = (cell / g.nc[2]) % g.nc[1];
+    int cx = cell / g.nyz;
+    bool fluid = (idt[i] & TYPE_BIT) == 0;
+    float ci = sound_speed(vi.w, ph);
+    float ax = 0.f, ay = 0.f, az = 0.f, dr = 0.f;
+    int zlo = max(cz - 1, 0), zhi = min(cz + 2, g.nc[2]);
+    for (int dx = -1; dx <= 1; ++dx) {
+        int x = cx + dx;
+        if (x < 0 || x >= g.nc[0]) continue;
+        for (int dy = -1; dy <= 1; ++dy) {
+            int y = cy + dy;
+            if (y < 0 || y >= g.nc[1]) continue;
+            uint32_t col = (uint32_t)(x * g.nc[1] + y) * g.nc[2];
+            uint32_t jb = cell_begin[col + zlo], je = cell_begin[col + zhi];
+            for (uint32_t j = jb; j < je; ++j) {
+                float4 pj = pos4[j];
+                float ddx = pi.x - pj.x, ddy = pi.y - pj.y, ddz = pi.z - pj.z;
+                float r2 = fmaf(ddz, ddz, fmaf(ddy, ddy, ddx * ddx));
+                if (r2 < ph.four_h2 && r2 > 0.0f) {
+                    float4 vj = velrho4[j];
+                    float mj = ph.uniform_mass ? ph.mass_fluid
+                                               : ((idt[j] & TYPE_BIT) ? ph.mass_bound : ph.mass_fluid);
+                    pair_term<KERNEL>(ddx, ddy, ddz, r2, vi.x, vi.y, vi.z, vi.w, pi.w, ci, vj, pj.w, mj, ph,
+                                      ax, ay, az, dr);
+                }
+            }
+        }
+    }
+    if (fluid) { ax += ph.g[0]; ay += ph.g[1]; az += ph.g[2]; }
+    else { ax = ay = az = 0.f; }
+    acc4[i] = make_float4(ax, ay, az, dr);
+}
+
+// ---- staged production kernel --------------------------------------------------------------------
+constexpr int IA_THREADS = 128;
+constexpr int IA_QCAP = 48;          // stack entries per thread
+constexpr int IA_SUB = 16;           // candidates tested between drain checks
+constexpr int IA_ZMAX = 32;          // max cells per z-block
+constexpr int IA_CAP = 1536;         // staged candidates per batch
+
+struct IaSmem {
+    float4 pos[IA_CAP];                       // x, y, z, p/rho^2
+    float4 vr[IA_CAP];                        // vx, vy, vz, rho
+    float mass[IA_CAP];                       // only written in the non-uniform-mass path
+    unsigned short stack[IA_QCAP * IA_THREADS];
+    uint32_t cbt[9][IA_ZMAX + 3];             // cell_begin of the 9 columns over [zlo, zhi]
+    uint32_t col_vstart[10];                  // virtual start of each column in the concatenation
+    uint32_t stage_lo[9], stage_hi[9];        // global index range of column staged in this batch
+    int32_t stage_off[9];                     // smem index = global index + stage_off
+};
+
+size_t interact_smem_bytes(const sph_ctx *) { return sizeof(IaSmem); }
+
+template <int KERNEL, bool UNIFORM>
+__global__ void __launch_bounds__(IA_THREADS)
+interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict__ velrho4,
+                       const uint32_t *__restrict__ idt, const uint32_t *__restrict__ keyword,
+                       const uint32_t *__restrict__ cell_begin, float4 *__restrict__ acc4,
+                       GridC g, PhysC ph, int zb, int nzb)
+{
+    extern __shared__ __align__(16) unsigned char ia_raw[];
+    IaSmem &S = *reinterpret_cast<IaSmem *>(ia_raw);
+    const int tid = threadIdx.x;
+
+    // ---- which z-block
+    uint32_t b = blockIdx.x;
+    const int bz = b % nzb;
+    b /= nzb;
+    const int cy = b % g.nc[1];
+    const int cx = b / g.nc[1];
+    const int cz0 = bz * zb, cz1 = min(cz0 + zb, g.nc[2]);
+    const uint32_t own_col = (uint32_t)(cx * g.nc[1] + cy) * g.nc[2];
+    const uint32_t t_begin = cell_begin[own_col + cz0], t_end = cell_begin[own_col + cz1];
+    if (t_begin == t_end) return;
+
+    const int zlo = max(cz0 - 1, 0), zhi = min(cz1 + 1, g.nc[2]);
+    const int nz = zhi - zlo;                                    // <= zb + 2
+    // ---- cell-begin table of the 9 columns
+    for (int k = tid; k < 9 * (nz + 1); k += IA_THREADS) {
+        int col = k / (nz + 1), z = k % (nz + 1);
+        int x = cx + col / 3 - 1, y = cy + col % 3 - 1;
+        uint32_t v = 0;
+        if (x >= 0 && x < g.nc[0] && y >= 0 && y < g.nc[1])
+            v = cell_begin[(uint32_t)(x * g.nc[1] + y) * g.nc[2] + zlo + z];
+        S.cbt[col][z] = v;          // columns outside the grid: all 0 => empty ranges
+    }
+    __syncthreads();
+    if (tid == 0) {
+        uint32_t acc = 0;
+        for (int col = 0; col < 9; ++col) {
+            S.col_vstart[col] = acc;
+            acc += S.cbt[col][nz] - S.cbt[col][0];
+        }
+        S.col_vstart[9] = acc;
+    }
+    __syncthreads();
+    const uint32_t total = S.col_vstart[9];
+    const uint32_t lane_full = 0xffffffffu;
+    unsigned short *stk = S.stack + tid;
+
+    for (uint32_t chunk = t_begin; chunk < t_end; chunk += IA_THREADS) {
+        const uint32_t i = chunk + tid;
+        const bool active = i < t_end;
+        float4 pi = make_float4(0.f, 0.f, 0.f, 0.f), vi = make_float4(0.f, 0.f, 0.f, 1.f);
+        int kz = 0;
+        bool fluid = false;
+        if (active) {
+            pi = pos4[i];
+            vi = velrho4[i];
+            fluid = (idt[i] & TYPE_BIT) == 0;
+            kz = (int)((keyword[i] & CELL_MASK) - own_col) - zlo;   // own cz - zlo
+        }
+        const float ci = sound_speed(vi.w, ph);
+        const int k_lo = max(kz - 1, 0), k_hi = min(kz + 2, nz);   // own 3-cell window in cbt rows
+        float ax = 0.f, ay = 0.f, az = 0.f, dr = 0.f;
+        int cnt = 0;
+
+        for (uint32_t bstart = 0; bstart < total; bstart += IA_CAP) {
+            const uint32_t bend = min(total, bstart + IA_CAP);
+            __syncthreads();                       // previous batch / chunk fully consumed
+            if (tid < 9) {
+                uint32_t vs = S.col_vstart[tid], ve = S.col_vstart[tid + 1];
+                uint32_t lo = max(vs, bstart), hi = min(ve, bend);
+                uint32_t gb = S.cbt[tid][0];
+                if (lo < hi) {
+                    S.stage_lo[tid] = gb + (lo - vs);
+                    S.stage_hi[tid] = gb + (hi - vs);
+                    S.stage_off[tid] = (int32_t)(lo - bstart) - (int32_t)(gb + (lo - vs));
+                } else {
+                    S.stage_lo[tid] = 0; S.stage_hi[tid] = 0; S.stage_off[tid] = 0;
+                }
+            }
+            __syncthreads();
+            // ---- stage: coalesced global reads, one column after the other
+            for (int col = 0; col < 9; ++col) {
+                const uint32_t lo = S.stage_lo[col], hi = S.stage_hi[col];
+                const int32_t off = S.stage_off[col];
+                for (uint32_t j = lo + tid; j < hi; j += IA_THREADS) {
+                    S.pos[(int32_t)j + off] = __ldg(pos4 + j);
+                    S.vr[(int32_t)j + off] = __ldg(velrho4 + j);
+                    if (!UNIFORM) S.mass[(int32_t)j + off] = (__ldg(idt + j) & TYPE_BIT) ? ph.mass_bound : ph.mass_fluid;
+                }
+            }
+            __syncthreads();
+
+            // ---- filter + drain
+            for (int col = 0; col < 9; ++col) {
+                int lo = 0, hi = 0;
+                if (active) {
+                    lo = (int)max(S.cbt[col][k_lo], S.stage_lo[col]);
+                    hi = (int)min(S.cbt[col][k_hi], S.stage_hi[col]);
+                }
+                const int off = S.stage_off[col];
+                const int len = max(hi - lo, 0);
+                const int maxlen = __reduce_max_sync(lane_full, len);
+                for (int sb = 0; sb < maxlen; sb += IA_SUB) {
+                    const int e = min(len, sb + IA_SUB);
+#pragma unroll 4
+                    for (int t = sb; t < e; ++t) {
+                        const int s = lo + t + off;
+                        const float4 pj = S.pos[s];
+                        const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
+                        const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+                        if (r2 < ph.four_h2 && r2 > 0.0f) {
+                            stk[cnt * IA_THREADS] = (unsigned short)s;
+                            ++cnt;
+                        }
+                    }
+                    while (__any_sync(lane_full, cnt > IA_QCAP - IA_SUB)) {
+                        if (cnt > 0) {
+                            --cnt;
+                            const int s = stk[cnt * IA_THREADS];
+                            const float4 pj = S.pos[s];
+                            const float4 vj = S.vr[s];
+                            const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
+                            const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+                            pair_term<KERNEL>(dx, dy, dz, r2, vi.x, vi.y, vi.z, vi.w, pi.w, ci, vj, pj.w,
+                                              UNIFORM ? 1.0f : S.mass[s], ph, ax, ay, az, dr);
+                        }
+                    }
+                }
+            }
+            // ---- flush the stacks before the staged data is replaced
+            while (__any_sync(lane_full, cnt > 0)) {
+                if (cnt > 0) {
+                    --cnt;
+                    const int s = stk[cnt * IA_THREADS];
+                    const float4 pj = S.pos[s];
+                    const float4 vj = S.vr[s];
+                    const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
+                    const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+                    pair_term<KERNEL>(dx, dy, dz, r2, vi.x, vi.y, vi.z, vi.w, pi.w, ci, vj, pj.w,
+                                      UNIFORM ? 1.0f : S.mass[s], ph, ax, ay, az, dr);
+                }
+            }
+        }
+        if (active) {
+            if (UNIFORM) { ax *= ph.mass_fluid; ay *= ph.mass_fluid; az *= ph.mass_fluid; dr *= ph.mass_fluid; }
+            if (fluid) { ax += ph.g[0]; ay += ph.g[1]; az += ph.g[2]; }
+            else { ax = ay = az = 0.f; }
+            acc4[i] = make_float4(ax, ay, az, dr);
+        }
+    }
+}
+
+template <int KERNEL, bool UNIFORM>
+static cudaError_t launch_staged(sph_ctx *c)
+{
+    auto kern = interact_staged_kernel<KERNEL, UNIFORM>;
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(IaSmem));
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    int zb = c->zblock;
+    int nzb = (c->grid.nc[2] + zb - 1) / zb;
+    uint64_t blocks = (uint64_t)c->grid.nc[0] * c->grid.nc[1] * nzb;
+    kern<<<(uint32_t)blocks, IA_THREADS, sizeof(IaSmem), c->stream>>>(
+        c->pos4[c->cur], c->velrho4[c->cur], c->idt[c->cur], c->keyword, c->cell_begin, c->acc4, c->grid,
+        c->phys, zb, nzb);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_interact(sph_ctx *c)
+{
+    uint32_t n = (uint32_t)c->n;
+    if (n == 0) return cudaSuccess;
+    const bool uni = c->phys.uniform_mass != 0;
+    if (c->interact_variant == 1) {
+        if (c->phys.kernel == 0)
+            interact_simple_kernel<0><<<(n + 127) / 128, 128, 0, c->stream>>>(
+                n, c->pos4[c->cur], c->velrho4[c->cur], c->idt[c->cur], c->keyword, c->cell_begin, c->acc4,
+                c->grid, c->phys);
+        else
+            interact_simple_kernel<1><<<(n + 127) / 128, 128, 0, c->stream>>>(
+                n, c->pos4[c->cur], c->velrho4[c->cur], c->idt[c->cur], c->keyword, c->cell_begin, c->acc4,
+                c->grid, c->phys);
+        return cudaGetLastError();
+    }
+    if (c->phys.kernel == 0) return uni ? launch_staged<0, true>(c) : launch_staged<0, false>(c);
+    return uni ? launch_staged<1, true>(c) : launch_staged<1, false>(c);
+}
+
+}  // namespace sph

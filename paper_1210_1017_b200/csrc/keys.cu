@@ -1,0 +1,160 @@
+// a1 - cell label + edge/migration tags per particle, scattered to id order, plus the digit
+// histograms of the radix sort ("a CUDA kernel is launched, with one thread per
+// particle, that assigns to each particle a label corresponding to the cell to which it
+// belongs"; L240 edge labels, L264 migration labels).
+//
+// HBM-bound: reads pos4 (16 B) + idt (4 B), writes one (keyword, value) pair (8 B) per
+// particle.  The pair is written at index id, so that the stable LSD sort that follows
+// starts from id order and ends in (cell, id) order whatever the previous order was.
+#include "sph_internal.cuh"
+
+namespace sph {
+
+// ---- state initialisation (id order) ----------------------------------------------------
+__global__ void init_state_kernel(uint32_t n, const float *__restrict__ pos, const float *__restrict__ vel,
+                                  const float *__restrict__ rho, const uint8_t *__restrict__ type,
+                                  float4 *__restrict__ pos4, float4 *__restrict__ velrho4,
+                                  float4 *__restrict__ velrhoM1, uint32_t *__restrict__ idt,
+                                  uint32_t *__restrict__ flags, PhysC ph)
+{
+    uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    float x = pos[3 * i], y = pos[3 * i + 1], z = pos[3 * i + 2];
+    float vx = vel[3 * i], vy = vel[3 * i + 1], vz = vel[3 * i + 2];
+    float r = rho[i];
+    if (!(isfinite(x) && isfinite(y) && isfinite(z) && isfinite(vx) && isfinite(vy) && isfinite(vz) &&
+          isfinite(r) && r > 0.f))
+        atomicOr(flags, FLAG_NONFINITE);
+    pos4[i] = make_float4(x, y, z, tait_p_over_rho2(r, ph));
+    float4 vr = make_float4(vx, vy, vz, r);
+    velrho4[i] = vr;
+    velrhoM1[i] = vr;
+    uint32_t t = type ? (type[i] ? TYPE_BIT : 0u) : 0u;
+    idt[i] = i | t;
+}
+
+cudaError_t launch_init_state(sph_ctx *c, const float *pos, const float *vel, const float *rho,
+                              const uint8_t *type)
+{
+    uint32_t n = (uint32_t)c->n;
+    if (n == 0) return cudaSuccess;
+    init_state_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(
+        n, pos, vel, rho, type, c->pos4[c->cur], c->velrho4[c->cur], c->velrhoM1[c->cur],
+        c->idt[c->cur], c->flags, c->phys);
+    return cudaGetLastError();
+}
+
+// ---- keys -----------------------------------------------------------------------------------
+__device__ __forceinline__ int cell_coord(float x, float mn, float inv, int nc)
+{
+    // one separately rounded fp32 subtract, one fp32 multiply, floor, clamp
+    float t = __fmul_rn(__fsub_rn(x, mn), inv);
+    int ci = __float2int_rd(t);           // floor; saturates for huge |t|
+    return min(max(ci, 0), nc - 1);
+}
+
+__device__ __forceinline__ int slab_of_plane(int cx, const SlabC &s)
+{
+    int k = 0;
+#pragma unroll
+    for (int j = 1; j < SPH_MAX_SLABS; ++j)
+        k += (j < s.n_slabs && cx >= s.planes[j]) ? 1 : 0;
+    return k;
+}
+
+__device__ __forceinline__ uint32_t edge_label(int cx, int slab, const SlabC &s)
+{
+    uint32_t lab = 0;
+    if (slab > 0 && cx == s.planes[slab]) lab = 1;
+    if (slab < s.n_slabs - 1 && cx == s.planes[slab + 1] - 1) lab = 2;
+    return lab;
+}
+
+// prev_mode: 0 = none (no migrants), 1 = previous slab ranges over the current order,
+//            2 = caller-supplied prev_init[id]
+template <int PASSES>
+__global__ void __launch_bounds__(256)
+keys_kernel(uint32_t n, const float4 *__restrict__ pos4, const uint32_t *__restrict__ idt,
+            uint2 *__restrict__ kv_by_id, uint32_t *__restrict__ hist, uint32_t *__restrict__ flags,
+            GridC g, SlabC sl, int prev_mode, int prev_n, const uint32_t *__restrict__ prev_slab_begin,
+            const uint8_t *__restrict__ prev_init)
+{
+    __shared__ uint32_t s_hist[PASSES * 256];
+    __shared__ uint32_t s_prev_begin[SPH_MAX_SLABS + 1];
+    for (int k = threadIdx.x; k < PASSES * 256; k += blockDim.x) s_hist[k] = 0;
+    if (prev_mode == 1 && threadIdx.x <= prev_n) s_prev_begin[threadIdx.x] = prev_slab_begin[threadIdx.x];
+    __syncthreads();
+
+    const uint32_t lane = threadIdx.x & 31;
+    const uint32_t lt_mask = (1u << lane) - 1u;
+    const uint32_t stride = gridDim.x * blockDim.x;
+    const uint32_t n_round = (n + 31u) & ~31u;    // keep warps converged for match_any
+    for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n_round; i += stride) {
+        bool valid = i < n;
+        uint32_t cell = 0;
+        if (valid) {
+            float4 p = pos4[i];
+            uint32_t w = idt[i];
+            uint32_t id = w & ID_MASK;
+            if (!(isfinite(p.x) && isfinite(p.y) && isfinite(p.z))) atomicOr(flags, FLAG_NONFINITE);
+            int cx = cell_coord(p.x, g.min[0], g.inv_cell, g.nc[0]);
+            int cy = cell_coord(p.y, g.min[1], g.inv_cell, g.nc[1]);
+            int cz = cell_coord(p.z, g.min[2], g.inv_cell, g.nc[2]);
+            cell = (uint32_t)((cx * g.nc[1] + cy) * g.nc[2] + cz);
+            int slab = slab_of_plane(cx, sl);
+            int prev = slab;
+            if (prev_mode == 1) {
+                prev = 0;
+#pragma unroll
+                for (int j = 1; j < SPH_MAX_SLABS; ++j)
+                    prev += (j < prev_n && i >= s_prev_begin[j]) ? 1 : 0;
+            } else if (prev_mode == 2) {
+                prev = min((int)prev_init[id], sl.n_slabs - 1);
+            }
+            uint32_t mig = slab < prev ? 1u : (slab > prev ? 2u : 0u);
+            uint32_t tag = edge_label(cx, slab, sl) | (mig << 2);
+            kv_by_id[id] = make_uint2((tag << TAG_SHIFT) | cell, ((uint32_t)prev << 28) | i);
+        }
+        // warp-aggregated digit histograms (one shared-memory atomic per distinct digit)
+#pragma unroll
+        for (int p = 0; p < PASSES; ++p) {
+            uint32_t d = valid ? ((cell >> (8 * p)) & 255u) : (256u + lane);
+            uint32_t m = __match_any_sync(0xffffffffu, d);
+            if (valid && (m & lt_mask) == 0) atomicAdd(&s_hist[p * 256 + d], __popc(m));
+        }
+    }
+    __syncthreads();
+    for (int k = threadIdx.x; k < PASSES * 256; k += blockDim.x) {
+        uint32_t v = s_hist[k];
+        if (v) atomicAdd(&hist[k], v);
+    }
+}
+
+cudaError_t launch_keys(sph_ctx *c)
+{
+    uint32_t n = (uint32_t)c->n;
+    cudaError_t e = cudaMemsetAsync(c->hist, 0, sizeof(uint32_t) * 256 * 4, c->stream);
+    if (e != cudaSuccess) return e;
+    if (n == 0) return cudaSuccess;
+    int prev_mode = c->have_prev_init ? 2 : (c->have_prev_ranges ? 1 : 0);
+    uint32_t blocks = (n + 255) / 256;
+    uint32_t cap = NUM_SMS * 8;
+    if (blocks > cap) blocks = cap;
+    const float4 *pos4 = c->pos4[c->cur];
+    const uint32_t *idt = c->idt[c->cur];
+    uint2 *kv = c->kv[0];
+#define SPH_KEYS(P)                                                                              \
+    keys_kernel<P><<<blocks, 256, 0, c->stream>>>(n, pos4, idt, kv, c->hist, c->flags, c->grid, \
+                                                  c->slabs, prev_mode, c->tagged_slabs.n_slabs, c->slab_begin, \
+                                                  c->prev_init)
+    switch (c->passes) {
+    case 1: SPH_KEYS(1); break;
+    case 2: SPH_KEYS(2); break;
+    case 3: SPH_KEYS(3); break;
+    default: SPH_KEYS(4); break;
+    }
+#undef SPH_KEYS
+    return cudaGetLastError();
+}
+
+}  // namespace sph

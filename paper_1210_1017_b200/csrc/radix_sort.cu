@@ -1,0 +1,193 @@
+// a2 - onesweep-style least-significant-digit radix sort of (keyword, value) pairs on the low
+// cell_bits of the keyword ("using the radix sort algorithm [18] to order the
+// array holding the particle identification labels, or IDs, according to the cell"; the paper's
+// three sorts per step - migration label L200, edge label L214, cell L220 - are one sort here,
+// the labels ride in the keyword's top bits).
+//
+// One kernel per 8-bit digit.  The digit histograms come from the key kernel (keys.cu); each
+// pass is a single sweep: a CTA takes a tile in launch order (dynamic tile id), ranks its keys
+// with warp-level match_any + per-warp shared-memory counters (stable), publishes its 256 digit
+// counts, resolves the exclusive prefix over earlier tiles by decoupled look-back, reorders the
+// tile through shared memory and writes runs of equal digits to consecutive addresses.
+//
+// HBM-bound: 8 B read + 8 B written per pair per pass.
+#include "sph_internal.cuh"
+
+namespace sph {
+
+constexpr int RS_THREADS = 512;
+constexpr int RS_IPT = 12;                        // pairs per thread
+constexpr int RS_TILE = RS_THREADS * RS_IPT;      // 6144 pairs = 48 KB staged
+constexpr int RS_WARPS = RS_THREADS / 32;
+constexpr uint32_t LB_AGG = 1u << 30;             // look-back word: flag in bits 30..31
+constexpr uint32_t LB_INC = 2u << 30;
+constexpr uint32_t LB_VAL = (1u << 30) - 1u;
+
+uint32_t radix_tiles(uint64_t n) { return (uint32_t)((n + RS_TILE - 1) / RS_TILE); }
+
+__device__ __forceinline__ uint32_t ld_relaxed(const uint32_t *p)
+{
+    uint32_t v;
+    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_relaxed(uint32_t *p, uint32_t v)
+{
+    asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+struct __align__(16) RsSmem {
+    uint2 stage[RS_TILE];                 // 48 KB
+    uint32_t warp_hist[RS_WARPS][256];    // 16 KB
+    uint32_t digit_start[256];            // first tile-local slot of each digit
+    uint32_t gbase[256];                  // global slot of tile-local slot 0 of each digit
+    uint32_t scan_tmp[16];
+    uint32_t tile;
+};
+
+__global__ void __launch_bounds__(RS_THREADS)
+onesweep_kernel(uint32_t n, const uint2 *__restrict__ in, uint2 *__restrict__ out,
+                const uint32_t *__restrict__ hist, uint32_t *tile_state, uint32_t *tile_counter, int shift,
+                uint32_t dmask /* keeps the tag bits 28..31 out of the last digit */)
+{
+    extern __shared__ __align__(16) unsigned char rs_raw[];
+    RsSmem &S = *reinterpret_cast<RsSmem *>(rs_raw);
+    const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t lt_mask = (1u << lane) - 1u;
+
+    if (tid == 0) S.tile = atomicAdd(tile_counter, 1u);
+    for (int k = tid; k < RS_WARPS * 256; k += RS_THREADS) (&S.warp_hist[0][0])[k] = 0;
+    __syncthreads();
+    const uint32_t tile = S.tile;
+    const uint32_t base = tile * RS_TILE;
+    const uint32_t tile_n = min((uint32_t)RS_TILE, n - base);
+
+    // ---- load, warp-striped: the warp owns a contiguous chunk; item k of lane l is chunk[k*32+l]
+    uint2 kv[RS_IPT];
+    uint32_t rank[RS_IPT];
+    const uint32_t wbase = warp * (32 * RS_IPT);
+#pragma unroll
+    for (int k = 0; k < RS_IPT; ++k) {
+        uint32_t li = wbase + k * 32 + lane;
+        kv[k] = li < tile_n ? __ldcs(in + base + li) : make_uint2(0xFFFFFFFFu, 0u);
+    }
+    // ---- rank inside the warp, stable in item order
+    uint32_t *wh = S.warp_hist[warp];
+#pragma unroll
+    for (int k = 0; k < RS_IPT; ++k) {
+        uint32_t li = wbase + k * 32 + lane;
+        bool valid = li < tile_n;
+        uint32_t d = valid ? ((kv[k].x >> shift) & dmask) : (256u + lane);
+        uint32_t m = __match_any_sync(0xffffffffu, d);
+        uint32_t leader = __ffs(m) - 1;
+        uint32_t old = 0;
+        if (valid && lane == leader) { old = wh[d]; wh[d] = old + __popc(m); }
+        old = __shfl_sync(0xffffffffu, old, leader);
+        rank[k] = old + __popc(m & lt_mask);
+        __syncwarp();
+    }
+    __syncthreads();
+
+    // ---- per digit (threads 0..255): scan over warps, publish, look back
+    uint32_t exc_in_warp = 0, hexc_in_warp = 0, lookback = 0;
+    if (tid < 256) {
+        uint32_t count = 0;
+#pragma unroll
+        for (int w = 0; w < RS_WARPS; ++w) {
+            uint32_t t = S.warp_hist[w][tid];
+            S.warp_hist[w][tid] = count;
+            count += t;
+        }
+        uint32_t *st = tile_state + (size_t)tile * 256 + tid;
+        st_relaxed(st, (tile == 0 ? LB_INC : LB_AGG) | count);     // publish first
+
+        uint32_t inc = count;                                       // tile counts over digits
+        uint32_t hcount = hist[tid], hinc = hcount;                 // whole-array counts over digits
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+            uint32_t u = __shfl_up_sync(0xffffffffu, hinc, o);
+            if (lane >= (uint32_t)o) { inc += t; hinc += u; }
+        }
+        if (lane == 31) { S.scan_tmp[warp] = inc; S.scan_tmp[8 + warp] = hinc; }
+        exc_in_warp = inc - count;
+        hexc_in_warp = hinc - hcount;
+
+        if (tile > 0) {                                             // same digit in earlier tiles
+            int t = (int)tile - 1;
+            while (true) {
+                uint32_t v = ld_relaxed(tile_state + (size_t)t * 256 + tid);
+                uint32_t f = v >> 30;
+                if (f == 0) continue;
+                lookback += v & LB_VAL;
+                if (f == 2) break;
+                --t;
+            }
+            st_relaxed(st, LB_INC | (lookback + count));
+        }
+    }
+    __syncthreads();
+    if (tid < 256) {
+        uint32_t add = 0, hadd = 0;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) {
+            add += (w < (int)warp) ? S.scan_tmp[w] : 0u;
+            hadd += (w < (int)warp) ? S.scan_tmp[8 + w] : 0u;
+        }
+        uint32_t dstart = exc_in_warp + add;
+        S.digit_start[tid] = dstart;
+        S.gbase[tid] = hexc_in_warp + hadd + lookback - dstart;
+    }
+    __syncthreads();
+
+    // ---- reorder the tile through shared memory
+#pragma unroll
+    for (int k = 0; k < RS_IPT; ++k) {
+        uint32_t li = wbase + k * 32 + lane;
+        if (li < tile_n) {
+            uint32_t d = (kv[k].x >> shift) & dmask;
+            S.stage[S.digit_start[d] + wh[d] + rank[k]] = kv[k];
+        }
+    }
+    __syncthreads();
+    // ---- runs of equal digits go to consecutive global addresses
+#pragma unroll
+    for (int k = 0; k < RS_IPT; ++k) {
+        uint32_t i = tid + k * RS_THREADS;
+        if (i < tile_n) {
+            uint2 e = S.stage[i];
+            uint32_t d = (e.x >> shift) & dmask;
+            out[S.gbase[d] + i] = e;
+        }
+    }
+}
+
+cudaError_t launch_sort(sph_ctx *c)
+{
+    uint32_t n = (uint32_t)c->n;
+    c->kv_sorted = c->passes & 1;
+    if (n == 0) return cudaSuccess;
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(onesweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             (int)sizeof(RsSmem));
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    uint32_t tiles = c->rs_tiles;
+    cudaError_t e = cudaMemsetAsync(c->tile_state, 0, sizeof(uint32_t) * 256 * (size_t)tiles * c->passes, c->stream);
+    if (e != cudaSuccess) return e;
+    e = cudaMemsetAsync(c->counters, 0, sizeof(uint32_t) * 64, c->stream);
+    if (e != cudaSuccess) return e;
+    for (int p = 0; p < c->passes; ++p) {
+        onesweep_kernel<<<tiles, RS_THREADS, sizeof(RsSmem), c->stream>>>(
+            n, c->kv[p & 1], c->kv[(p + 1) & 1], c->hist + 256 * p,
+            c->tile_state + (size_t)p * tiles * 256, c->counters + p, 8 * p,
+            (CELL_MASK >> (8 * p)) & 255u);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
+}
+
+}  // namespace sph

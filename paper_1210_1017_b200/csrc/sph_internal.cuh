@@ -1,0 +1,143 @@
+// Internal declarations shared by the translation units of libsph_b200.so.
+// Nothing here is part of the ABI (include/sph_b200.h is).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "sph_b200.h"
+
+namespace sph {
+
+constexpr uint32_t CELL_MASK = 0x0FFFFFFFu;   // keyword bits 0..27 = cell label
+constexpr int TAG_SHIFT = 28;                 // bits 28..29 edge label, 30..31 migration label
+constexpr uint32_t ID_MASK = 0x0FFFFFFFu;     // idt bits 0..27 = id, bit 31 = type
+constexpr uint32_t TYPE_BIT = 0x80000000u;
+constexpr int NUM_SMS = 148;                  // B200
+
+// sticky device flags
+constexpr uint32_t FLAG_NONFINITE = 1u;
+
+// ---- constants handed to kernels by value -------------------------------------------
+struct GridC {
+    float min[3];
+    float inv_cell;          // 1.0f / (2.0f * h), one fp32 op each (key arithmetic)
+    int nc[3];
+    int nyz;                 // nc[1]*nc[2]
+    uint32_t ncells;
+};
+
+struct SlabC {
+    int n_slabs;
+    int planes[SPH_MAX_SLABS + 1];
+};
+
+struct PhysC {
+    float h, inv_h_half;     // 0.5/h
+    float four_h2;           // (2h)^2
+    float eta2;              // 0.01 h^2
+    float kF;                // Wendland: -5 aD / h^2 ; cubic spline: aD / h^2 (see interact.cu)
+    float alpha_h;           // alpha * h
+    float rho0, inv_rho0, c0, B;
+    float tait[16];          // binomial coefficients C(gamma, k), k = 1..gamma
+    int gamma;
+    float g[3];
+    float mass_fluid, mass_bound;
+    int uniform_mass;
+    int kernel;
+};
+
+// ---- profiling ------------------------------------------------------------------------
+struct StageTimer {
+    static constexpr int MAX_PAIRS = 4096;
+    cudaEvent_t ev[2 * MAX_PAIRS];
+    int stage[MAX_PAIRS];
+    int n_pairs = 0;
+    int n_created = 0;
+    bool enabled = false;
+};
+
+}  // namespace sph
+
+struct sph_ctx {
+    sph_params P;
+    sph::GridC grid;
+    sph::SlabC slabs;          // planes used by the next sort
+    sph::SlabC tagged_slabs;   // planes the last sort (or retag) labelled with
+    sph::PhysC phys;
+    uint64_t n;
+    int max_slabs;
+    int cell_bits, passes;
+    cudaStream_t stream;
+    int sticky;                // SPH_OK or SPH_ERR_CUDA
+
+    // state (double-buffered for the permutation); cur = live buffer
+    float4 *pos4[2], *velrho4[2], *velrhoM1[2];
+    uint32_t *idt[2];
+    int cur;
+    float4 *acc4;
+    // sort
+    uint2 *kv[2];              // (keyword, prevSlab<<28 | sourceIndex)
+    int kv_sorted;             // which kv buffer holds the sorted pairs
+    uint32_t *keyword;         // sorted keywords
+    uint32_t *hist;            // passes*256 digit histograms
+    uint32_t *tile_state;      // passes * rs_tiles * 256 look-back words
+    uint32_t *counters;        // 64 words: dynamic tile counters, scan tickets
+    uint32_t rs_tiles;
+    // cells / slabs
+    uint32_t *cell_begin;      // ncells+1
+    unsigned long long *scan_state;   // look-back words of the cell fill and migrant scans
+    uint32_t scan_tiles_cells, scan_tiles_mig;
+    uint32_t *slab_begin;      // max_slabs+1 (current), also "previous owner" ranges of the next sort
+    uint32_t *halo_range;      // 2*max_slabs * 2 (begin, count)
+    uint32_t *halo_offset;     // 2*max_slabs+1
+    float4 *halo_pos4, *halo_velrho4;
+    uint32_t *halo_idt;
+    uint4 *migrants;
+    uint32_t *mig_total, *mig_count;
+    uint8_t *prev_init;        // n bytes: caller-supplied previous owner for the first sort
+    uint32_t *flags;           // sticky device flags
+
+    bool have_prev_init;       // prev_init valid for the next sort
+    bool have_prev_ranges;     // slab_begin valid as previous-owner ranges
+    bool sorted_valid;         // arrays sorted + cell table valid for the current positions
+    bool halos_valid;
+    bool rates_valid;
+    uint64_t step_index;
+    int interact_variant;
+    int zblock;                // cells per z-block of the staged interaction kernel
+
+    sph::StageTimer timer;
+};
+
+namespace sph {
+
+// every launcher enqueues on ctx->stream and returns a cudaError_t
+cudaError_t launch_init_state(sph_ctx *c, const float *pos, const float *vel, const float *rho,
+                              const uint8_t *type);
+cudaError_t launch_keys(sph_ctx *c);
+cudaError_t launch_sort(sph_ctx *c);
+cudaError_t launch_gather_cells(sph_ctx *c);
+cudaError_t launch_cell_fill(sph_ctx *c);
+cudaError_t launch_slab_meta(sph_ctx *c);
+cudaError_t launch_retag(sph_ctx *c);
+cudaError_t launch_halo_gather(sph_ctx *c);
+cudaError_t launch_migrants(sph_ctx *c);
+cudaError_t launch_interact(sph_ctx *c);
+cudaError_t launch_verlet(sph_ctx *c, float dt, int corrective);
+cudaError_t launch_download_pack(sph_ctx *c, float *pos3, float *vel3, float *rho, float *acc3,
+                                 float *drho);
+
+uint32_t radix_tiles(uint64_t n);
+uint32_t scan_tiles(uint64_t n);
+size_t interact_smem_bytes(const sph_ctx *c);
+
+// Tait pressure over rho^2 from rho, fp32, cancellation-free.
+__device__ __forceinline__ float tait_p_over_rho2(float rho, const PhysC &ph)
+{
+    float d = (rho - ph.rho0) * ph.inv_rho0;        // delta = rho/rho0 - 1, subtraction exact near rho0
+    float s = ph.tait[ph.gamma];                    // Horner over sum_k C(gamma,k) delta^k
+    for (int k = ph.gamma - 1; k >= 1; --k) s = fmaf(s, d, ph.tait[k]);
+    float p = ph.B * d * s;
+    return __fdividef(p, rho * rho);
+}
+
+}  // namespace sph

@@ -1,0 +1,84 @@
+// a8 - system update ("the system state can be updated by numerical
+// integration ... here a second-order Verlet algorithm is used"; L116: for dynamic boundary
+// particles "the integration update for position and velocity is not performed").
+// Formulas are reading A7 of DESIGN.md:
+//   ordinary step     v+ = v(n-1) + 2 dt a,  rho+ = rho(n-1) + 2 dt drho
+//   corrective step   v+ = v + dt a,         rho+ = rho + dt drho        (step 0 and every Ns-th)
+//   always            r+ = r + dt v + dt^2 a / 2 ;  (v, rho)(n-1) <- (v, rho)
+// The new p/rho^2 (Tait, L112) is stored with the position for the next interaction pass.
+// HBM-bound: 68 B read + 48 B written per particle.  Also holds the id-order download pack.
+#include "sph_internal.cuh"
+
+namespace sph {
+
+__global__ void __launch_bounds__(256)
+verlet_kernel(uint32_t n, float4 *__restrict__ pos4, float4 *__restrict__ velrho4,
+              float4 *__restrict__ velrhoM1, const float4 *__restrict__ acc4,
+              const uint32_t *__restrict__ idt, uint32_t *__restrict__ flags, PhysC ph, float dt,
+              int corrective)
+{
+    uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    float4 p = pos4[i];
+    float4 v = velrho4[i];
+    float4 m = velrhoM1[i];
+    float4 a = __ldcs(acc4 + i);
+    const bool fluid = (idt[i] & TYPE_BIT) == 0;
+    const float dt2 = dt + dt, hdt2 = 0.5f * dt * dt;
+    float rho_new = corrective ? fmaf(dt, a.w, v.w) : fmaf(dt2, a.w, m.w);
+    float4 vn = v;
+    if (fluid) {
+        vn.x = corrective ? fmaf(dt, a.x, v.x) : fmaf(dt2, a.x, m.x);
+        vn.y = corrective ? fmaf(dt, a.y, v.y) : fmaf(dt2, a.y, m.y);
+        vn.z = corrective ? fmaf(dt, a.z, v.z) : fmaf(dt2, a.z, m.z);
+        p.x = fmaf(hdt2, a.x, fmaf(dt, v.x, p.x));
+        p.y = fmaf(hdt2, a.y, fmaf(dt, v.y, p.y));
+        p.z = fmaf(hdt2, a.z, fmaf(dt, v.z, p.z));
+    }
+    vn.w = rho_new;
+    if (!(isfinite(p.x) && isfinite(p.y) && isfinite(p.z) && isfinite(rho_new) && rho_new > 0.f))
+        atomicOr(flags, FLAG_NONFINITE);
+    p.w = tait_p_over_rho2(rho_new, ph);
+    pos4[i] = p;
+    velrho4[i] = vn;
+    velrhoM1[i] = v;
+}
+
+cudaError_t launch_verlet(sph_ctx *c, float dt, int corrective)
+{
+    uint32_t n = (uint32_t)c->n;
+    if (n == 0) return cudaSuccess;
+    verlet_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(n, c->pos4[c->cur], c->velrho4[c->cur],
+                                                        c->velrhoM1[c->cur], c->acc4, c->idt[c->cur],
+                                                        c->flags, c->phys, dt, corrective);
+    return cudaGetLastError();
+}
+
+// ---- download: scatter to id order into packed staging arrays ----------------------------------
+__global__ void __launch_bounds__(256)
+download_pack_kernel(uint32_t n, const float4 *__restrict__ pos4, const float4 *__restrict__ velrho4,
+                     const float4 *__restrict__ acc4, const uint32_t *__restrict__ idt,
+                     float *__restrict__ pos3, float *__restrict__ vel3, float *__restrict__ rho,
+                     float *__restrict__ acc3, float *__restrict__ drho)
+{
+    uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    uint32_t id = idt[i] & ID_MASK;
+    float4 p = pos4[i], v = velrho4[i], a = acc4[i];
+    if (pos3) { pos3[3 * id] = p.x; pos3[3 * id + 1] = p.y; pos3[3 * id + 2] = p.z; }
+    if (vel3) { vel3[3 * id] = v.x; vel3[3 * id + 1] = v.y; vel3[3 * id + 2] = v.z; }
+    if (rho) rho[id] = v.w;
+    if (acc3) { acc3[3 * id] = a.x; acc3[3 * id + 1] = a.y; acc3[3 * id + 2] = a.z; }
+    if (drho) drho[id] = a.w;
+}
+
+cudaError_t launch_download_pack(sph_ctx *c, float *pos3, float *vel3, float *rho, float *acc3, float *drho)
+{
+    uint32_t n = (uint32_t)c->n;
+    if (n == 0) return cudaSuccess;
+    download_pack_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(n, c->pos4[c->cur], c->velrho4[c->cur], c->acc4,
+                                                               c->idt[c->cur], pos3, vel3, rho, acc3, drho);
+    return cudaGetLastError();
+}
+
+}  // namespace sph
