@@ -1,0 +1,375 @@
+#!/usr/bin/env python
+"""bench.py - whole-hot-path throughput of the B200 SPH step (BASELINE.json metric:
+Mparticle-steps/s on synthetic 3-D dam breaks, radix-sort Gkeys/s, % of roofline).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 0..3] [--impl reference]
+    python bench.py --micro 26            # sort/halo microbenchmark at N = 2^26 (configs[4])
+
+One "step" = one sph_step() = all rows of the hot path (keys+tags, radix sort, payload
+permutation, cell table, halo gather, migrant compaction, 27-cell interaction, Verlet) over the
+whole particle set.  Default workload: BASELINE config 3 (32 M fluid + 2 M boundary particles,
+16 logical x-slabs), the size the roofline bars are judged at; its working set (6.5 GB) is far
+larger than the 126 MB L2, so no L2 flush is needed between steps.
+
+N > 1 (torchrun): the path has no inter-GPU exchange (BASELINE north_star drops it), so every
+rank steps an independent replica ("replicas only", weak scaling); time = max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+CONFIG_NB = {0: 16, 1: 100, 2: 200, 3: 317}
+METRIC = "Mparticle-steps/s"
+FP32_LANES_PER_SM, NUM_SMS = 128, 148
+FLOPS_PER_CANDIDATE, FLOPS_PER_PAIR = 8, 32
+# algorithmic HBM bytes per particle of the memory-bound stages
+BYTES = dict(keys=28.0, sort_per_pass=16.0, gather=116.0, verlet=116.0, migrate=4.0)
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        d = json.load(open(path))
+        return dict(hbm_gbs=float(d["hbm_gbs"]), sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)), source="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+class ClockSampler:
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.idx = gpu_index
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+
+    def start(self):
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(self.idx), f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self) -> dict:
+        if self.p is None:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
+        time.sleep(0.15)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, reasons, power = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f:
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 9:
+                continue
+            try:
+                sm.append(float(c[1])); mx.append(float(c[2])); power.append(float(c[3]))
+            except ValueError:
+                continue
+            for k, nm in enumerate(names):
+                if c[5 + k].lower().startswith("active"):
+                    reasons.add(nm)
+        self.f.close()
+        os.unlink(self.f.name)
+        if not sm:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["no samples"])
+        return dict(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), reasons=sorted(reasons),
+                    power_w_max=float(max(power)), samples=len(sm))
+
+
+def oracle_step_sample(w, max_particles: int):
+    """Time the oracles, as they stand, on a bounded spatial sample of the workload: the
+    particles with the smallest x (a contiguous piece of the tank, boundary included).
+    Returns (particles, seconds, cores, description)."""
+    from oracle import physics as OB
+    from oracle import structure as OA
+    n = min(w.n, max_particles)
+    if n < w.n:
+        xs = np.partition(w.pos[:, 0], n - 1)[n - 1]
+        sel = np.nonzero(w.pos[:, 0] <= xs)[0][:n]
+    else:
+        sel = np.arange(w.n)
+    pos, vel, rho, typ = w.pos[sel], w.vel[sel], w.rho[sel], w.type[sel]
+    P = w.params
+    p = OB.params_from_workload(P)
+    OB.lib()
+    s = OB.State(pos, vel, rho, typ)
+    nc = OA.grid_dims(P["dom_min"], P["dom_max"], P["h"])
+    from paper_1210_1017_b200 import workloads as W
+    planes = W.slab_planes(nc[0], w.n_slabs)
+    t0 = time.perf_counter()
+    OA.structure(pos, np.arange(len(sel)), P["dom_min"], P["dom_max"], P["h"], planes)
+    OB.step(p, s, w.dt, verlet_ns=P["verlet_ns"])
+    dt = time.perf_counter() - t0
+    return len(sel), dt, OB.threads(), f"{len(sel)} particles of lowest x of {w.name}, 1 step (structure + rates + Verlet)"
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle, as it stands, on a bounded sample per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_1210_1017_b200 import workloads as W
+    nb = CONFIG_NB[args.config]
+    w = W.dam_break(nb)
+    budget = args.ref_sample
+    n_s, _, cores, desc = oracle_step_sample(w, budget)           # warm-up (builds the library)
+    for _ in range(max(0, args.warmup - 1)):
+        oracle_step_sample(w, budget)
+    t = 0.0
+    for _ in range(args.steps):
+        _, dt, _, _ = oracle_step_sample(w, budget)
+        t += dt
+    value = n_s * args.steps / t / 1e6
+    line = dict(impl="reference", metric=METRIC, value=value, unit="Mparticle-steps/s", n_gpus=args.gpus,
+                steps=args.steps, warmup=args.warmup, ms_per_step=1e3 * t / args.steps,
+                higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64", data="synthetic",
+                config=dict(workload=f"config{args.config}: {w.name}", n_particles=w.n, n_slabs=w.n_slabs,
+                            sample=desc),
+                cpu_baseline=dict(value=value, unit="Mparticle-steps/s", cores=cores, kind="oracle", sample=desc),
+                e2e=dict(value=value, unit="Mparticle-steps/s", h2d_bytes_per_step=0, d2h_bytes_per_step=0),
+                gpu_launches=0)
+    print(json.dumps(line))
+
+
+def run_micro(args):
+    """Sort/halo microbenchmark (configs[4]); prints its own JSON (not the driver's line)."""
+    import torch
+    from paper_1210_1017_b200 import binding as B
+    from paper_1210_1017_b200 import workloads as W
+    n = 1 << args.micro
+    w = W.uniform_cube(n)
+    pk = peaks()
+    sph = B.Sph(w.params, w.pos, w.vel, w.rho, w.type, prev_slab=w.prev_slab)
+    v = sph.sph_get_view()
+    planes = W.slab_planes(v.nc[0], 8)
+    sph.sph_set_slabs(planes)
+    dpos = torch.from_numpy(w.pos).cuda()
+    dvel = torch.from_numpy(w.vel).cuda()
+    drho = torch.from_numpy(w.rho).cuda()
+    dprev = torch.from_numpy(w.prev_slab).cuda()
+    reps = args.steps
+    acc = {}
+    for it in range(args.warmup + reps):
+        sph.sph_set_state(dpos, dvel, drho, None, dprev)          # restore random order (untimed)
+        sph.sph_profile_enable(it >= args.warmup)
+        sph.sph_sort_and_cells()
+        sph.sph_build_halos()
+        if it >= args.warmup:
+            for k, (ms, c) in sph.sph_profile_read().items():
+                acc.setdefault(k, []).append(ms)
+    T = sph.view_tensors()
+    n_halo = int(T["halo_offset"][-1].item())
+    n_mig = int(T["mig_total"].item())
+    passes = (v.cell_bits + 7) // 8
+    med = {k: float(np.median(x)) for k, x in acc.items() if np.sum(x) > 0}
+    byts = dict(keys=BYTES["keys"] * n, sort=BYTES["sort_per_pass"] * passes * n, gather=BYTES["gather"] * n,
+                cells=8.0 * (v.ncells + 1), halo=72.0 * n_halo, migrate=4.0 * n + 16.0 * n_mig)
+    out = dict(workload=w.name, n=n, cell_bits=v.cell_bits, passes=passes, n_halo=n_halo, n_migrants=n_mig,
+               sort_gkeys_s=n / (med["sort"] * 1e-3) / 1e9,
+               sort_with_keys_gkeys_s=n / ((med["sort"] + med["keys"]) * 1e-3) / 1e9,
+               hbm_peak_gbs=pk["hbm_gbs"], peak_source=pk["source"],
+               stages={k: dict(ms=med[k], algorithmic_gbs=byts[k] / (med[k] * 1e-3) / 1e9,
+                               frac_of_hbm_peak=byts[k] / (med[k] * 1e-3) / 1e9 / pk["hbm_gbs"])
+                       for k in med if k in byts})
+    print(json.dumps(out))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=None)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--config", type=int, default=3, choices=[0, 1, 2, 3])
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--micro", type=int, default=0, help="log2 N of the sort/halo microbenchmark")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--cpu-sample", type=int, default=1_500_000, help="particles of the cpu_baseline sample")
+    ap.add_argument("--ref-sample", type=int, default=300_000, help="particles per step of --impl reference")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--variant", type=int, default=0)
+    args = ap.parse_args()
+    if args.steps is None:
+        args.steps = 10 if (args.impl == "reference" or args.micro) else {0: 200, 1: 200, 2: 200, 3: 100}[args.config]
+    args.warmup = max(args.warmup, 3)
+
+    if args.impl == "reference":
+        run_reference(args)
+        return
+    if args.micro:
+        run_micro(args)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_1210_1017_b200 import binding as B      # fails loudly without the CUDA library
+    from paper_1210_1017_b200 import workloads as W
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    pk = peaks()
+
+    nb = CONFIG_NB[args.config]
+    w = W.dam_break(nb)
+    sph = B.Sph(w.params, w.pos, w.vel, w.rho, w.type, device=f"cuda:{local}")
+    sph.sph_set_option(B.SPH_OPT_INTERACT_VARIANT, args.variant)
+    v = sph.sph_get_view()
+    planes = W.slab_planes(v.nc[0], w.n_slabs)
+    sph.sph_set_slabs(planes)
+    n = w.n
+    passes = (v.cell_bits + 7) // 8
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    # ---- warm-up
+    for _ in range(args.warmup):
+        sph.sph_step(w.dt)
+    assert sph.sph_status() == 0
+    # pair statistics of the state the timed region starts from (for the flop count)
+    sph.sph_sort_and_cells()
+    cand, pairs = sph.sph_pair_stats()
+    launches0 = sph.sph_launch_count()
+
+    # ---- timed region: exactly K steps, device-timed, stage timers on the same stream
+    sampler = ClockSampler(local)
+    sph.sph_profile_enable(True)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    sampler.start()
+    ev0.record()
+    for _ in range(args.steps):
+        sph.sph_step(w.dt)
+    ev1.record()
+    barrier()
+    clocks = sampler.stop()
+    ms_total = ev0.elapsed_time(ev1)
+    stage = sph.sph_profile_read()
+    sph.sph_profile_enable(False)
+    launches = sph.sph_launch_count() - launches0
+    assert sph.sph_status() == 0, "non-finite state during the timed run"
+    if world > 1:
+        t = torch.tensor([ms_total], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    value = world * n * args.steps / (ms_total * 1e-3) / 1e6
+
+    # ---- end-to-end through the C ABI with HOST buffers: upload, step, download, every step
+    pin = dict(pos=torch.from_numpy(w.pos).pin_memory(), vel=torch.from_numpy(w.vel).pin_memory(),
+               rho=torch.from_numpy(w.rho).pin_memory(), typ=torch.from_numpy(w.type).pin_memory())
+    outp = dict(pos=torch.empty((n, 3), dtype=torch.float32).pin_memory(),
+                vel=torch.empty((n, 3), dtype=torch.float32).pin_memory(),
+                rho=torch.empty(n, dtype=torch.float32).pin_memory())
+
+    def e2e_step():
+        sph.sph_set_state(pin["pos"].numpy(), pin["vel"].numpy(), pin["rho"].numpy(), pin["typ"].numpy())
+        sph.sph_step(w.dt)
+        sph.sph_download(acc=False, drho=False, pinned=outp)
+
+    if args.e2e_steps > 0:
+        e2e_step()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.e2e_steps):
+        e2e_step()
+    torch.cuda.synchronize()
+    e2e_s = max(time.perf_counter() - t0, 1e-9)
+    if world > 1:
+        t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    e2e = dict(value=world * n * args.e2e_steps / e2e_s / 1e6, unit="Mparticle-steps/s",
+               h2d_bytes_per_step=int(n * (12 + 12 + 4 + 1)), d2h_bytes_per_step=int(n * (12 + 12 + 4)),
+               steps=args.e2e_steps, api="sph_set_state(host) + sph_step + sph_download(host), pinned buffers")
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (interaction): plain FP32 ALUs
+    ia_ms, ia_n = stage["interact"]
+    ia_ms_avg = ia_ms / max(ia_n, 1)
+    flops = FLOPS_PER_CANDIDATE * cand + FLOPS_PER_PAIR * pairs
+    achieved = flops / (ia_ms_avg * 1e-3) / 1e12
+    peak = NUM_SMS * FP32_LANES_PER_SM * 2 * pk["sm_max_mhz"] * 1e6 / 1e12
+    sm_mhz = clocks.get("sm_mhz") or pk["sm_max_mhz"]
+    roofline = dict(bound="alu", kernel="interact_staged_kernel", achieved=achieved, peak=peak, unit="TFLOP/s",
+                    frac=achieved / peak, traffic=None,
+                    peak_source=f"148 SMs x 128 FP32 lanes x 2 flop x {pk['sm_max_mhz']:.0f} MHz (max clock, {pk['source']})",
+                    frac_at_observed_clock=achieved / (peak * sm_mhz / pk["sm_max_mhz"]),
+                    algorithmic_flops_per_launch=flops, candidates=cand, pairs=pairs,
+                    avg_launch_ms=ia_ms_avg, share_of_step=ia_ms / ms_total)
+
+    T = sph.view_tensors()
+    n_halo = int(T["halo_offset"][-1].item()) if w.n_slabs > 1 else 0
+    n_mig = int(T["mig_total"].item())
+    byts = dict(keys=BYTES["keys"] * n, sort=BYTES["sort_per_pass"] * passes * n, gather=BYTES["gather"] * n,
+                cells=8.0 * (v.ncells + 1), halo=72.0 * n_halo, migrate=4.0 * n + 16.0 * n_mig,
+                verlet=BYTES["verlet"] * n)
+    stages = {}
+    for k, (ms, c) in stage.items():
+        if c == 0:
+            continue
+        avg = ms / c
+        d = dict(ms=avg, share=ms / ms_total)
+        if k in byts:
+            gbs = byts[k] / (avg * 1e-3) / 1e9
+            d.update(algorithmic_gbs=gbs, frac_of_hbm_peak=gbs / pk["hbm_gbs"])
+        stages[k] = d
+
+    cpu = None
+    if not args.no_cpu_baseline:
+        oracle_step_sample(w, 20_000)                         # builds / warms the oracle library
+        n_s, dt_s, cores, desc = oracle_step_sample(w, args.cpu_sample)
+        cpu = dict(value=n_s / dt_s / 1e6, unit="Mparticle-steps/s", cores=cores, kind="oracle", sample=desc,
+                   seconds=dt_s)
+
+    line = dict(
+        metric=METRIC, value=value, unit="Mparticle-steps/s", n_gpus=world, steps=args.steps, warmup=args.warmup,
+        ms_per_step=ms_total / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32",
+        data="synthetic",
+        config=dict(workload=f"config{args.config}: 3-D dam break, {w.n_fluid} fluid + {n - w.n_fluid} boundary "
+                             f"particles, {w.n_slabs} logical x-slabs",
+                    n_particles=n, n_slabs=w.n_slabs, cells=int(v.ncells), cell_bits=int(v.cell_bits),
+                    radix_passes=passes, dt=w.dt, multi_gpu="replicas only",
+                    l2="no flush: per-step working set %.1f GB >> 126 MB L2" % (n * 250e-9)
+                    if n > 5_000_000 else "working set fits L2 (small config)"),
+        clocks=clocks, e2e=e2e, gpu_launches=int(launches), roofline=roofline, cpu_baseline=cpu,
+        sort_gkeys_s=n / (stages["sort"]["ms"] * 1e-3) / 1e9 if "sort" in stages else None,
+        stages=stages, hbm_peak_gbs=pk["hbm_gbs"], peak_source=pk["source"])
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -175,6 +175,13 @@ int sph_set_option(sph_ctx *ctx, int option, int value);
 int sph_profile_enable(sph_ctx *ctx, int enable);
 int sph_profile_read(sph_ctx *ctx, float *ms, int *launches);
 
+/* Measurement helpers (not on the hot path).  sph_pair_stats: runs a counting kernel over the
+ * current sorted state and returns, in HOST out[2], the number of candidate pairs the 27-cell
+ * search examines and the number of pairs inside the support (0 < r < 2h); synchronises.
+ * sph_launch_count: HOST *out = number of kernels this context has launched so far. */
+int sph_pair_stats(sph_ctx *ctx, uint64_t *out);
+int sph_launch_count(const sph_ctx *ctx, uint64_t *out);
+
 void sph_destroy(sph_ctx *ctx);
 const char *sph_strerror(int code);
 

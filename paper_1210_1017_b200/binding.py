@@ -30,7 +30,7 @@ SPH_OPT_INTERACT_VARIANT = 0
 EXPORTS = ["sph_workspace_bytes", "sph_init", "sph_set_state", "sph_set_slabs", "sph_slab_planes_from_x",
            "sph_sort_and_cells", "sph_build_halos", "sph_interact", "sph_step", "sph_get_view",
            "sph_download", "sph_status", "sph_set_option", "sph_profile_enable", "sph_profile_read",
-           "sph_destroy", "sph_strerror"]
+           "sph_pair_stats", "sph_launch_count", "sph_destroy", "sph_strerror"]
 
 
 class sph_params(C.Structure):
@@ -84,6 +84,10 @@ _lib.sph_profile_enable.restype = C.c_int
 _lib.sph_profile_enable.argtypes = [C.c_void_p, C.c_int]
 _lib.sph_profile_read.restype = C.c_int
 _lib.sph_profile_read.argtypes = [C.c_void_p, C.POINTER(C.c_float), C.POINTER(C.c_int)]
+_lib.sph_pair_stats.restype = C.c_int
+_lib.sph_pair_stats.argtypes = [C.c_void_p, C.POINTER(C.c_uint64)]
+_lib.sph_launch_count.restype = C.c_int
+_lib.sph_launch_count.argtypes = [C.c_void_p, C.POINTER(C.c_uint64)]
 _lib.sph_destroy.restype = None
 _lib.sph_destroy.argtypes = [C.c_void_p]
 _lib.sph_strerror.restype = C.c_char_p
@@ -228,6 +232,17 @@ class Sph:
         cnt = (C.c_int * SPH_T_COUNT)()
         _check(_lib.sph_profile_read(self._ctx, ms, cnt))
         return {STAGE_NAMES[k]: (float(ms[k]), int(cnt[k])) for k in range(SPH_T_COUNT)}
+
+    def sph_pair_stats(self):
+        """(candidate pairs examined by the 27-cell search, pairs with 0 < r < 2h)."""
+        out = (C.c_uint64 * 2)()
+        _check(_lib.sph_pair_stats(self._ctx, out))
+        return int(out[0]), int(out[1])
+
+    def sph_launch_count(self) -> int:
+        out = C.c_uint64(0)
+        _check(_lib.sph_launch_count(self._ctx, C.byref(out)))
+        return int(out.value)
 
     def sph_get_view(self) -> sph_view:
         v = sph_view()

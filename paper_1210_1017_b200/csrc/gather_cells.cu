@@ -51,6 +51,7 @@ cudaError_t launch_gather_cells(sph_ctx *c)
         gather_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(
             n, c->kv[c->kv_sorted], c->pos4[c->cur], c->velrho4[c->cur], c->velrhoM1[c->cur], c->idt[c->cur],
             c->pos4[o], c->velrho4[o], c->velrhoM1[o], c->idt[o], c->keyword, c->cell_begin);
+        c->n_launches++;
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;
         c->cur = o;
@@ -155,6 +156,7 @@ cudaError_t launch_cell_fill(sph_ctx *c)
     if (e != cudaSuccess) return e;
     cell_fill_kernel<<<tiles, CF_THREADS, 0, c->stream>>>(m, (uint32_t)c->n, c->cell_begin, c->scan_state,
                                                         c->counters + 8);
+    c->n_launches++;
     return cudaGetLastError();
 }
 
@@ -197,6 +199,7 @@ cudaError_t launch_slab_meta(sph_ctx *c)
 {
     slab_meta_kernel<<<1, 64, 0, c->stream>>>(c->cell_begin, c->tagged_slabs, c->grid.nyz, c->slab_begin,
                                               c->halo_range, c->halo_offset, c->mig_total, c->mig_count);
+    c->n_launches++;
     return cudaGetLastError();
 }
 
@@ -221,6 +224,7 @@ cudaError_t launch_retag(sph_ctx *c)
     uint32_t n = (uint32_t)c->n;
     if (n == 0) return cudaSuccess;
     retag_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(n, c->keyword, c->tagged_slabs, c->grid.nyz);
+    c->n_launches++;
     return cudaGetLastError();
 }
 

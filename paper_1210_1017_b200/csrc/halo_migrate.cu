@@ -42,6 +42,7 @@ cudaError_t launch_halo_gather(sph_ctx *c)
     halo_gather_kernel<<<grid, 256, 0, c->stream>>>(c->halo_range, c->halo_offset, c->pos4[c->cur],
                                                     c->velrho4[c->cur], c->idt[c->cur], c->halo_pos4,
                                                     c->halo_velrho4, c->halo_idt);
+    c->n_launches++;
     return cudaGetLastError();
 }
 
@@ -144,6 +145,7 @@ cudaError_t launch_migrants(sph_ctx *c)
     migrants_kernel<<<tiles, MG_THREADS, 0, c->stream>>>(
         n, c->keyword, c->kv[c->kv_sorted], c->idt[c->cur], c->tagged_slabs, c->grid.nyz, c->scan_state,
         c->counters + 9, c->migrants, c->mig_total, c->mig_count);
+    c->n_launches++;
     return cudaGetLastError();
 }
 

@@ -119,27 +119,44 @@ interact_simple_kernel(uint32_t n, const float4 *__restrict__ pos4, const float4
 }
 
 // ---- staged production kernel --------------------------------------------------------------------
-constexpr int IA_THREADS = 128;
+constexpr int IA_THREADS = 256;
 constexpr int IA_QCAP = 48;          // stack entries per thread
 constexpr int IA_SUB = 16;           // candidates tested between drain checks
 constexpr int IA_ZMAX = 32;          // max cells per z-block
-constexpr int IA_CAP = 1536;         // staged candidates per batch
+constexpr int IA_CAP = 2688;         // staged candidates per batch (9 columns x 11 cells x 27 + slack)
+constexpr float IA_TINY = 1e-30f;    // r2 floor: a coincident pair (the particle itself) adds exactly 0
 
 struct IaSmem {
     float4 pos[IA_CAP];                       // x, y, z, p/rho^2
-    float4 vr[IA_CAP];                        // vx, vy, vz, rho
-    float mass[IA_CAP];                       // only written in the non-uniform-mass path
-    unsigned short stack[IA_QCAP * IA_THREADS];
+    float4 vr[IA_CAP];                        // vx, vy, vz, rho (sign bit = boundary type if masses differ)
+    unsigned short stack[IA_QCAP * IA_THREADS];   // [entry][thread]: byte offset of a candidate in pos[]/vr[]
     uint32_t cbt[9][IA_ZMAX + 3];             // cell_begin of the 9 columns over [zlo, zhi]
     uint32_t col_vstart[10];                  // virtual start of each column in the concatenation
-    uint32_t stage_lo[9], stage_hi[9];        // global index range of column staged in this batch
+    uint32_t stage_lo[9], stage_hi[9];        // global index range of the column staged in this batch
     int32_t stage_off[9];                     // smem index = global index + stage_off
 };
 
 size_t interact_smem_bytes(const sph_ctx *) { return sizeof(IaSmem); }
 
+__device__ __forceinline__ void sts_u16(uint32_t addr, uint32_t v)
+{
+    asm volatile("st.shared.u16 [%0], %1;" ::"r"(addr), "h"((unsigned short)v) : "memory");
+}
+__device__ __forceinline__ uint32_t lds_u16(uint32_t addr)
+{
+    unsigned short v;
+    asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(addr) : "memory");
+    return v;
+}
+__device__ __forceinline__ float4 lds_f4(uint32_t addr)
+{
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+    return v;
+}
+
 template <int KERNEL, bool UNIFORM>
-__global__ void __launch_bounds__(IA_THREADS)
+__global__ void __launch_bounds__(IA_THREADS, 2)
 interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict__ velrho4,
                        const uint32_t *__restrict__ idt, const uint32_t *__restrict__ keyword,
                        const uint32_t *__restrict__ cell_begin, float4 *__restrict__ acc4,
@@ -183,7 +200,11 @@ interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict
     __syncthreads();
     const uint32_t total = S.col_vstart[9];
     const uint32_t lane_full = 0xffffffffu;
-    unsigned short *stk = S.stack + tid;
+    const uint32_t pos_base = (uint32_t)__cvta_generic_to_shared(S.pos);
+    const uint32_t vr_delta = (uint32_t)__cvta_generic_to_shared(S.vr) - pos_base;
+    const uint32_t stk_base = (uint32_t)__cvta_generic_to_shared(S.stack) + 2u * tid;
+    constexpr uint32_t STK_STRIDE = 2u * IA_THREADS;
+    const uint32_t stk_high = stk_base + STK_STRIDE * (IA_QCAP - IA_SUB);
 
     for (uint32_t chunk = t_begin; chunk < t_end; chunk += IA_THREADS) {
         const uint32_t i = chunk + tid;
@@ -200,7 +221,24 @@ interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict
         const float ci = sound_speed(vi.w, ph);
         const int k_lo = max(kz - 1, 0), k_hi = min(kz + 2, nz);   // own 3-cell window in cbt rows
         float ax = 0.f, ay = 0.f, az = 0.f, dr = 0.f;
-        int cnt = 0;
+        uint32_t sp = stk_base;                                     // shared address of the stack top
+
+        auto drain_one = [&]() {
+            if (sp > stk_base) {
+                sp -= STK_STRIDE;
+                const uint32_t o = lds_u16(sp);
+                const float4 pj = lds_f4(pos_base + o);
+                float4 vj = lds_f4(pos_base + vr_delta + o);
+                const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
+                const float r2 = fmaxf(fmaf(dz, dz, fmaf(dy, dy, dx * dx)), IA_TINY);
+                float mj = 1.0f;
+                if (!UNIFORM) {
+                    mj = vj.w < 0.f ? ph.mass_bound : ph.mass_fluid;
+                    vj.w = fabsf(vj.w);
+                }
+                pair_term<KERNEL>(dx, dy, dz, r2, vi.x, vi.y, vi.z, vi.w, pi.w, ci, vj, pj.w, mj, ph, ax, ay, az, dr);
+            }
+        };
 
         for (uint32_t bstart = 0; bstart < total; bstart += IA_CAP) {
             const uint32_t bend = min(total, bstart + IA_CAP);
@@ -224,8 +262,9 @@ interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict
                 const int32_t off = S.stage_off[col];
                 for (uint32_t j = lo + tid; j < hi; j += IA_THREADS) {
                     S.pos[(int32_t)j + off] = __ldg(pos4 + j);
-                    S.vr[(int32_t)j + off] = __ldg(velrho4 + j);
-                    if (!UNIFORM) S.mass[(int32_t)j + off] = (__ldg(idt + j) & TYPE_BIT) ? ph.mass_bound : ph.mass_fluid;
+                    float4 v = __ldg(velrho4 + j);
+                    if (!UNIFORM && (__ldg(idt + j) & TYPE_BIT)) v.w = -v.w;
+                    S.vr[(int32_t)j + off] = v;
                 }
             }
             __syncthreads();
@@ -240,46 +279,26 @@ interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict
                 const int off = S.stage_off[col];
                 const int len = max(hi - lo, 0);
                 const int maxlen = __reduce_max_sync(lane_full, len);
-                for (int sb = 0; sb < maxlen; sb += IA_SUB) {
-                    const int e = min(len, sb + IA_SUB);
-#pragma unroll 4
-                    for (int t = sb; t < e; ++t) {
-                        const int s = lo + t + off;
-                        const float4 pj = S.pos[s];
+                // byte offsets into pos[]: candidate t of this lane is at o_lo + 16 t, valid while < o_hi
+                uint32_t o = (uint32_t)(lo + off) * 16u;
+                const uint32_t o_hi = o + (uint32_t)len * 16u;
+                for (int sb = 0; sb < maxlen; sb += IA_SUB, o += 16u * IA_SUB) {
+#pragma unroll
+                    for (int u = 0; u < IA_SUB; ++u) {
+                        const uint32_t ou = o + 16u * u;
+                        const bool in = ou < o_hi;
+                        const float4 pj = lds_f4(pos_base + (in ? ou : 0u));
                         const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
                         const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                        if (r2 < ph.four_h2 && r2 > 0.0f) {
-                            stk[cnt * IA_THREADS] = (unsigned short)s;
-                            ++cnt;
-                        }
+                        const bool hit = in && (r2 < ph.four_h2);
+                        if (hit) sts_u16(sp, ou);
+                        sp += hit ? STK_STRIDE : 0u;
                     }
-                    while (__any_sync(lane_full, cnt > IA_QCAP - IA_SUB)) {
-                        if (cnt > 0) {
-                            --cnt;
-                            const int s = stk[cnt * IA_THREADS];
-                            const float4 pj = S.pos[s];
-                            const float4 vj = S.vr[s];
-                            const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
-                            const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                            pair_term<KERNEL>(dx, dy, dz, r2, vi.x, vi.y, vi.z, vi.w, pi.w, ci, vj, pj.w,
-                                              UNIFORM ? 1.0f : S.mass[s], ph, ax, ay, az, dr);
-                        }
-                    }
+                    while (__any_sync(lane_full, sp > stk_high)) drain_one();
                 }
             }
             // ---- flush the stacks before the staged data is replaced
-            while (__any_sync(lane_full, cnt > 0)) {
-                if (cnt > 0) {
-                    --cnt;
-                    const int s = stk[cnt * IA_THREADS];
-                    const float4 pj = S.pos[s];
-                    const float4 vj = S.vr[s];
-                    const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
-                    const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                    pair_term<KERNEL>(dx, dy, dz, r2, vi.x, vi.y, vi.z, vi.w, pi.w, ci, vj, pj.w,
-                                      UNIFORM ? 1.0f : S.mass[s], ph, ax, ay, az, dr);
-                }
-            }
+            while (__any_sync(lane_full, sp > stk_base)) drain_one();
         }
         if (active) {
             if (UNIFORM) { ax *= ph.mass_fluid; ay *= ph.mass_fluid; az *= ph.mass_fluid; dr *= ph.mass_fluid; }
@@ -306,6 +325,51 @@ static cudaError_t launch_staged(sph_ctx *c)
     kern<<<(uint32_t)blocks, IA_THREADS, sizeof(IaSmem), c->stream>>>(
         c->pos4[c->cur], c->velrho4[c->cur], c->idt[c->cur], c->keyword, c->cell_begin, c->acc4, c->grid,
         c->phys, zb, nzb);
+    c->n_launches++;
+    return cudaGetLastError();
+}
+
+// ---- measurement helper: candidate and neighbour pair counts -----------------------------------
+__global__ void __launch_bounds__(128)
+pair_stats_kernel(uint32_t n, const float4 *__restrict__ pos4, const uint32_t *__restrict__ keyword,
+                  const uint32_t *__restrict__ cell_begin, GridC g, float four_h2, unsigned long long *out)
+{
+    uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned long long cand = 0, acc = 0;
+    if (i < n) {
+        float4 pi = pos4[i];
+        uint32_t cell = keyword[i] & CELL_MASK;
+        int cz = cell % g.nc[2], cy = (cell / g.nc[2]) % g.nc[1], cx = cell / g.nyz;
+        int zlo = max(cz - 1, 0), zhi = min(cz + 2, g.nc[2]);
+        for (int dx = -1; dx <= 1; ++dx)
+            for (int dy = -1; dy <= 1; ++dy) {
+                int x = cx + dx, y = cy + dy;
+                if (x < 0 || x >= g.nc[0] || y < 0 || y >= g.nc[1]) continue;
+                uint32_t col = (uint32_t)(x * g.nc[1] + y) * g.nc[2];
+                uint32_t jb = cell_begin[col + zlo], je = cell_begin[col + zhi];
+                cand += je - jb;
+                for (uint32_t j = jb; j < je; ++j) {
+                    float4 pj = pos4[j];
+                    float ddx = pi.x - pj.x, ddy = pi.y - pj.y, ddz = pi.z - pj.z;
+                    float r2 = fmaf(ddz, ddz, fmaf(ddy, ddy, ddx * ddx));
+                    acc += (r2 < four_h2 && r2 > 0.0f) ? 1 : 0;
+                }
+            }
+    }
+    for (int o = 16; o; o >>= 1) {
+        cand += __shfl_xor_sync(0xffffffffu, cand, o);
+        acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    }
+    if ((threadIdx.x & 31) == 0) { atomicAdd(out, cand); atomicAdd(out + 1, acc); }
+}
+
+cudaError_t launch_pair_stats(sph_ctx *c, unsigned long long *d_out)
+{
+    uint32_t n = (uint32_t)c->n;
+    cudaError_t e = cudaMemsetAsync(d_out, 0, 16, c->stream);
+    if (e != cudaSuccess || n == 0) return e;
+    pair_stats_kernel<<<(n + 127) / 128, 128, 0, c->stream>>>(n, c->pos4[c->cur], c->keyword, c->cell_begin,
+                                                             c->grid, c->phys.four_h2, d_out);
     return cudaGetLastError();
 }
 
@@ -323,7 +387,8 @@ cudaError_t launch_interact(sph_ctx *c)
             interact_simple_kernel<1><<<(n + 127) / 128, 128, 0, c->stream>>>(
                 n, c->pos4[c->cur], c->velrho4[c->cur], c->idt[c->cur], c->keyword, c->cell_begin, c->acc4,
                 c->grid, c->phys);
-        return cudaGetLastError();
+        c->n_launches++;
+    return cudaGetLastError();
     }
     if (c->phys.kernel == 0) return uni ? launch_staged<0, true>(c) : launch_staged<0, false>(c);
     return uni ? launch_staged<1, true>(c) : launch_staged<1, false>(c);

@@ -41,6 +41,7 @@ cudaError_t launch_init_state(sph_ctx *c, const float *pos, const float *vel, co
     init_state_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(
         n, pos, vel, rho, type, c->pos4[c->cur], c->velrho4[c->cur], c->velrhoM1[c->cur],
         c->idt[c->cur], c->flags, c->phys);
+    c->n_launches++;
     return cudaGetLastError();
 }
 
@@ -154,6 +155,7 @@ cudaError_t launch_keys(sph_ctx *c)
     default: SPH_KEYS(4); break;
     }
 #undef SPH_KEYS
+    c->n_launches++;
     return cudaGetLastError();
 }
 

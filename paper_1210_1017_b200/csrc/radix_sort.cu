@@ -184,6 +184,7 @@ cudaError_t launch_sort(sph_ctx *c)
             n, c->kv[p & 1], c->kv[(p + 1) & 1], c->hist + 256 * p,
             c->tile_state + (size_t)p * tiles * 256, c->counters + p, 8 * p,
             (CELL_MASK >> (8 * p)) & 255u);
+        c->n_launches++;
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }

@@ -282,9 +282,9 @@ int sph_init(sph_ctx **out, const sph_params *p, const sph_particles *part, int 
     c->prev_init = (uint8_t *)(w + L.prev_init);
     c->flags = (uint32_t *)(w + L.flags);
     c->interact_variant = 0;
-    // cells per z-block of the interaction kernel: fill the 128-thread CTA with targets
+    // cells per z-block of the interaction kernel: fill the 256-thread CTA with targets
     double ppc = pow(2.0 * (double)p->h / (double)p->dp, 3.0);
-    int zb = (int)floor(128.0 * 0.97 / (ppc > 0.05 ? ppc : 0.05));
+    int zb = (int)floor(256.0 * 0.97 / (ppc > 0.05 ? ppc : 0.05));
     if (zb < 1) zb = 1;
     if (zb > 32) zb = 32;
     c->zblock = zb;
@@ -517,6 +517,28 @@ int sph_profile_read(sph_ctx *c, float *ms, int *launches)
         }
     }
     t.n_pairs = 0;
+    return SPH_OK;
+}
+
+int sph_pair_stats(sph_ctx *c, uint64_t *out)
+{
+    if (!c || !out) return SPH_ERR_ARG;
+    if (c->sticky) return c->sticky;
+    if (!c->sorted_valid) return SPH_ERR_ORDER;
+    unsigned long long *d = c->scan_state;          // idle between calls
+    CK(c, launch_pair_stats(c, d));
+    unsigned long long h[2] = {0, 0};
+    CK(c, cudaMemcpyAsync(h, d, 16, cudaMemcpyDeviceToHost, c->stream));
+    CK(c, cudaStreamSynchronize(c->stream));
+    out[0] = h[0];
+    out[1] = h[1];
+    return SPH_OK;
+}
+
+int sph_launch_count(const sph_ctx *c, uint64_t *out)
+{
+    if (!c || !out) return SPH_ERR_ARG;
+    *out = c->n_launches;
     return SPH_OK;
 }
 

@@ -47,7 +47,7 @@ struct PhysC {
 
 // ---- profiling ------------------------------------------------------------------------
 struct StageTimer {
-    static constexpr int MAX_PAIRS = 4096;
+    static constexpr int MAX_PAIRS = 16384;
     cudaEvent_t ev[2 * MAX_PAIRS];
     int stage[MAX_PAIRS];
     int n_pairs = 0;
@@ -105,6 +105,8 @@ struct sph_ctx {
     int interact_variant;
     int zblock;                // cells per z-block of the staged interaction kernel
 
+    uint64_t n_launches;       // kernels launched so far (memsets and copies not counted)
+
     sph::StageTimer timer;
 };
 
@@ -123,6 +125,7 @@ cudaError_t launch_halo_gather(sph_ctx *c);
 cudaError_t launch_migrants(sph_ctx *c);
 cudaError_t launch_interact(sph_ctx *c);
 cudaError_t launch_verlet(sph_ctx *c, float dt, int corrective);
+cudaError_t launch_pair_stats(sph_ctx *c, unsigned long long *d_out);
 cudaError_t launch_download_pack(sph_ctx *c, float *pos3, float *vel3, float *rho, float *acc3,
                                  float *drho);
 

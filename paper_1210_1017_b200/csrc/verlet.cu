@@ -51,6 +51,7 @@ cudaError_t launch_verlet(sph_ctx *c, float dt, int corrective)
     verlet_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(n, c->pos4[c->cur], c->velrho4[c->cur],
                                                         c->velrhoM1[c->cur], c->acc4, c->idt[c->cur],
                                                         c->flags, c->phys, dt, corrective);
+    c->n_launches++;
     return cudaGetLastError();
 }
 
@@ -78,6 +79,7 @@ cudaError_t launch_download_pack(sph_ctx *c, float *pos3, float *vel3, float *rh
     if (n == 0) return cudaSuccess;
     download_pack_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(n, c->pos4[c->cur], c->velrho4[c->cur], c->acc4,
                                                                c->idt[c->cur], pos3, vel3, rho, acc3, drho);
+    c->n_launches++;
     return cudaGetLastError();
 }
 
