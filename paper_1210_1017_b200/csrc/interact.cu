@@ -120,8 +120,8 @@ interact_simple_kernel(uint32_t n, const float4 *__restrict__ pos4, const float4
 
 // ---- staged production kernel --------------------------------------------------------------------
 constexpr int IA_THREADS = 256;
-constexpr int IA_QCAP = 48;          // stack entries per thread
-constexpr int IA_SUB = 16;           // candidates tested between drain checks
+constexpr int IA_QCAP = 24;          // stack entries per thread; one entry = 16 candidates' hit mask
+constexpr int IA_SUB = 16;           // candidates tested per stack entry
 constexpr int IA_ZMAX = 32;          // max cells per z-block
 constexpr int IA_CAP = 2688;         // staged candidates per batch (9 columns x 11 cells x 27 + slack)
 constexpr float IA_TINY = 1e-30f;    // r2 floor: a coincident pair (the particle itself) adds exactly 0
@@ -129,7 +129,7 @@ constexpr float IA_TINY = 1e-30f;    // r2 floor: a coincident pair (the particl
 struct IaSmem {
     float4 pos[IA_CAP];                       // x, y, z, p/rho^2
     float4 vr[IA_CAP];                        // vx, vy, vz, rho (sign bit = boundary type if masses differ)
-    unsigned short stack[IA_QCAP * IA_THREADS];   // [entry][thread]: byte offset of a candidate in pos[]/vr[]
+    uint32_t stack[IA_QCAP * IA_THREADS];     // [entry][thread]: byte offset of 16 candidates << 16 | hit mask
     uint32_t cbt[9][IA_ZMAX + 3];             // cell_begin of the 9 columns over [zlo, zhi]
     uint32_t col_vstart[10];                  // virtual start of each column in the concatenation
     uint32_t stage_lo[9], stage_hi[9];        // global index range of the column staged in this batch
@@ -138,14 +138,14 @@ struct IaSmem {
 
 size_t interact_smem_bytes(const sph_ctx *) { return sizeof(IaSmem); }
 
-__device__ __forceinline__ void sts_u16(uint32_t addr, uint32_t v)
+__device__ __forceinline__ void sts_u32(uint32_t addr, uint32_t v)
 {
-    asm volatile("st.shared.u16 [%0], %1;" ::"r"(addr), "h"((unsigned short)v) : "memory");
+    asm volatile("st.shared.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
 }
-__device__ __forceinline__ uint32_t lds_u16(uint32_t addr)
+__device__ __forceinline__ uint32_t lds_u32(uint32_t addr)
 {
-    unsigned short v;
-    asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(addr) : "memory");
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
     return v;
 }
 __device__ __forceinline__ float4 lds_f4(uint32_t addr)
@@ -202,9 +202,9 @@ interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict
     const uint32_t lane_full = 0xffffffffu;
     const uint32_t pos_base = (uint32_t)__cvta_generic_to_shared(S.pos);
     const uint32_t vr_delta = (uint32_t)__cvta_generic_to_shared(S.vr) - pos_base;
-    const uint32_t stk_base = (uint32_t)__cvta_generic_to_shared(S.stack) + 2u * tid;
-    constexpr uint32_t STK_STRIDE = 2u * IA_THREADS;
-    const uint32_t stk_high = stk_base + STK_STRIDE * (IA_QCAP - IA_SUB);
+    const uint32_t stk_base = (uint32_t)__cvta_generic_to_shared(S.stack) + 4u * tid;
+    constexpr uint32_t STK_STRIDE = 4u * IA_THREADS;
+    const uint32_t stk_high = stk_base + STK_STRIDE * (IA_QCAP - 2);
 
     for (uint32_t chunk = t_begin; chunk < t_end; chunk += IA_THREADS) {
         const uint32_t i = chunk + tid;
@@ -223,10 +223,18 @@ interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict
         float ax = 0.f, ay = 0.f, az = 0.f, dr = 0.f;
         uint32_t sp = stk_base;                                     // shared address of the stack top
 
+        uint32_t cur_mask = 0, cur_o = 0;                          // entry being drained
         auto drain_one = [&]() {
-            if (sp > stk_base) {
+            if (cur_mask == 0 && sp > stk_base) {
                 sp -= STK_STRIDE;
-                const uint32_t o = lds_u16(sp);
+                const uint32_t e = lds_u32(sp);
+                cur_mask = e & 0xFFFFu;
+                cur_o = e >> 16;
+            }
+            if (cur_mask) {
+                const uint32_t bit = __ffs(cur_mask) - 1;
+                cur_mask &= cur_mask - 1;
+                const uint32_t o = cur_o + 16u * bit;
                 const float4 pj = lds_f4(pos_base + o);
                 float4 vj = lds_f4(pos_base + vr_delta + o);
                 const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
@@ -279,26 +287,44 @@ interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict
                 const int off = S.stage_off[col];
                 const int len = max(hi - lo, 0);
                 const int maxlen = __reduce_max_sync(lane_full, len);
-                // byte offsets into pos[]: candidate t of this lane is at o_lo + 16 t, valid while < o_hi
-                uint32_t o = (uint32_t)(lo + off) * 16u;
+                // lanes without work in this column read from offset 0 and record nothing
+                const bool work = len > 0;
+                const int minlen = __reduce_min_sync(lane_full, work ? len : 0x7fffffff);
+                // byte offsets into pos[]: candidate t of this lane is at o + 16 t, valid while < o_hi
+                uint32_t o = work ? (uint32_t)(lo + off) * 16u : 0u;
                 const uint32_t o_hi = o + (uint32_t)len * 16u;
-                for (int sb = 0; sb < maxlen; sb += IA_SUB, o += 16u * IA_SUB) {
+                int sb = 0;
+                // sub-batches of 16 that are complete for every working lane: no range checks
+                for (; sb + IA_SUB <= minlen && sb < maxlen; sb += IA_SUB, o += 16u * IA_SUB) {
+                    uint32_t mask = 0;
 #pragma unroll
                     for (int u = 0; u < IA_SUB; ++u) {
-                        const uint32_t ou = o + 16u * u;
-                        const bool in = ou < o_hi;
-                        const float4 pj = lds_f4(pos_base + (in ? ou : 0u));
+                        const float4 pj = lds_f4(pos_base + o + 16u * u);
                         const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
                         const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                        const bool hit = in && (r2 < ph.four_h2);
-                        if (hit) sts_u16(sp, ou);
-                        sp += hit ? STK_STRIDE : 0u;
+                        if (r2 < ph.four_h2) mask |= 1u << u;
                     }
+                    if (work && mask) { sts_u32(sp, (o << 16) | mask); sp += STK_STRIDE; }
+                    while (__any_sync(lane_full, sp > stk_high)) drain_one();
+                }
+                // ragged remainder in groups of 4 with per-lane range checks (reads past o_hi stay
+                // inside the CTA's shared memory: o < 16 IA_CAP and advances by at most 16 IA_CAP)
+                for (; sb < maxlen; sb += 4, o += 64u) {
+                    uint32_t mask = 0;
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const uint32_t ou = o + 16u * u;
+                        const float4 pj = lds_f4(pos_base + ou);
+                        const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
+                        const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+                        if (ou < o_hi && r2 < ph.four_h2) mask |= 1u << u;
+                    }
+                    if (mask) { sts_u32(sp, (o << 16) | mask); sp += STK_STRIDE; }
                     while (__any_sync(lane_full, sp > stk_high)) drain_one();
                 }
             }
             // ---- flush the stacks before the staged data is replaced
-            while (__any_sync(lane_full, sp > stk_base)) drain_one();
+            while (__any_sync(lane_full, (sp > stk_base) || cur_mask != 0)) drain_one();
         }
         if (active) {
             if (UNIFORM) { ax *= ph.mass_fluid; ay *= ph.mass_fluid; az *= ph.mass_fluid; dr *= ph.mass_fluid; }
