@@ -24,33 +24,48 @@
 namespace sph {
 
 // ---- pair term ---------------------------------------------------------------------------------
-// Returns F with grad_i W_ij = F r_ij, for 0 < r2 < 4h^2.
+__device__ __forceinline__ float rsqrt_fast(float x)        // 1 MUFU, |rel err| <= 2^-22
+{
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float rcp_fast(float x)          // 1 MUFU, |rel err| <= 2^-23
+{
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// Returns F with grad_i W_ij = F r_ij, for 0 < r2 (F -> 0 smoothly at r = 2h and is clamped to
+// 0 beyond, so a filter that lets a pair marginally outside 2h through changes nothing).
 template <int KERNEL>
 __device__ __forceinline__ float kernel_F(float r2, const PhysC &ph)
 {
-    float rinv = rsqrtf(r2);
+    float rinv = rsqrt_fast(r2);
     float r = r2 * rinv;
     if (KERNEL == 0) {                      // Wendland C2: F = -5 aD (1 - q/2)^3 / h^2
-        float t = fmaf(-ph.inv_h_half, r, 1.0f);
+        float t = fmaxf(fmaf(-ph.inv_h_half, r, 1.0f), 0.0f);
         return ph.kF * t * t * t;
     } else {                                // cubic spline, kF = aD / h^2
         float q = r * (2.0f * ph.inv_h_half);
-        float t = 2.0f - q;
+        float t = fmaxf(2.0f - q, 0.0f);
         float f = q <= 1.0f ? fmaf(2.25f, q, -3.0f) : -0.75f * t * t * rinv * ph.h;
         return ph.kF * f;
     }
 }
 
+template <bool GAMMA7>
 __device__ __forceinline__ float sound_speed(float rho, const PhysC &ph)
 {
     float x = rho * ph.inv_rho0;
-    if (ph.gamma == 7) return ph.c0 * x * x * x;
+    if (GAMMA7) return ph.c0 * x * x * x;               // c0 (rho/rho0)^((gamma-1)/2), gamma = 7
     return ph.c0 * __powf(x, 0.5f * (float)(ph.gamma - 1));
 }
 
 // Adds the contribution of neighbour j to (ax, ay, az, dr); masses are applied by the caller
-// (mj = 1 in the uniform-mass path).
-template <int KERNEL>
+// (mj = 1 in the uniform-mass path).  Branch-free: the viscous term uses min(v_ij.r_ij, 0).
+template <int KERNEL, bool GAMMA7>
 __device__ __forceinline__ void pair_term(float dx, float dy, float dz, float r2,
                                           float vxi, float vyi, float vzi, float rhoi, float Pi_, float ci,
                                           float4 vj, float Pj, float mj, const PhysC &ph,
@@ -60,12 +75,9 @@ __device__ __forceinline__ void pair_term(float dx, float dy, float dz, float r2
     float dvx = vxi - vj.x, dvy = vyi - vj.y, dvz = vzi - vj.z;
     float dot = fmaf(dvz, dz, fmaf(dvy, dy, dvx * dx));
     dr = fmaf(F, dot, dr);                                            // Eq. (7)
-    float visc = 0.0f;
-    if (dot < 0.0f) {                                                 // L112
-        float cj = sound_speed(vj.w, ph);
-        // Pi = -alpha cbar mu / rhobar = -alpha h (ci+cj) dot / ((r2+eta2)(rhoi+rhoj))
-        visc = -ph.alpha_h * (ci + cj) * dot * __frcp_rn((r2 + ph.eta2) * (rhoi + vj.w));
-    }
+    // L112: Pi = -alpha cbar mu / rhobar = -alpha h (ci+cj) dot / ((r2+eta2)(rhoi+rhoj)) if dot < 0
+    float cj = sound_speed<GAMMA7>(vj.w, ph);
+    float visc = -ph.alpha_h * (ci + cj) * fminf(dot, 0.0f) * rcp_fast((r2 + ph.eta2) * (rhoi + vj.w));
     float coef = -F * (Pi_ + Pj + visc);                              // Eq. (9)
     ax = fmaf(coef, dx, ax);
     ay = fmaf(coef, dy, ay);
@@ -73,7 +85,7 @@ __device__ __forceinline__ void pair_term(float dx, float dy, float dz, float r2
 }
 
 // ---- simple cross-check kernel -----------------------------------------------------------------
-template <int KERNEL>
+template <int KERNEL, bool GAMMA7>
 __global__ void __launch_bounds__(128)
 interact_simple_kernel(uint32_t n, const float4 *__restrict__ pos4, const float4 *__restrict__ velrho4,
                        const uint32_t *__restrict__ idt, const uint32_t *__restrict__ keyword,
@@ -88,7 +100,7 @@ interact_simple_kernel(uint32_t n, const float4 *__restrict__ pos4, const float4
     int cy = (cell / g.nc[2]) % g.nc[1];
     int cx = cell / g.nyz;
     bool fluid = (idt[i] & TYPE_BIT) == 0;
-    float ci = sound_speed(vi.w, ph);
+    float ci = sound_speed<GAMMA7>(vi.w, ph);
     float ax = 0.f, ay = 0.f, az = 0.f, dr = 0.f;
     int zlo = max(cz - 1, 0), zhi = min(cz + 2, g.nc[2]);
     for (int dx = -1; dx <= 1; ++dx) {
@@ -107,7 +119,7 @@ interact_simple_kernel(uint32_t n, const float4 *__restrict__ pos4, const float4
                     float4 vj = velrho4[j];
                     float mj = ph.uniform_mass ? ph.mass_fluid
                                                : ((idt[j] & TYPE_BIT) ? ph.mass_bound : ph.mass_fluid);
-                    pair_term<KERNEL>(ddx, ddy, ddz, r2, vi.x, vi.y, vi.z, vi.w, pi.w, ci, vj, pj.w, mj, ph,
+                    pair_term<KERNEL, GAMMA7>(ddx, ddy, ddz, r2, vi.x, vi.y, vi.z, vi.w, pi.w, ci, vj, pj.w, mj, ph,
                                       ax, ay, az, dr);
                 }
             }
@@ -155,7 +167,7 @@ __device__ __forceinline__ float4 lds_f4(uint32_t addr)
     return v;
 }
 
-template <int KERNEL, bool UNIFORM>
+template <int KERNEL, bool UNIFORM, bool GAMMA7>
 __global__ void __launch_bounds__(IA_THREADS, 2)
 interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict__ velrho4,
                        const uint32_t *__restrict__ idt, const uint32_t *__restrict__ keyword,
@@ -218,7 +230,7 @@ interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict
             fluid = (idt[i] & TYPE_BIT) == 0;
             kz = (int)((keyword[i] & CELL_MASK) - own_col) - zlo;   // own cz - zlo
         }
-        const float ci = sound_speed(vi.w, ph);
+        const float ci = sound_speed<GAMMA7>(vi.w, ph);
         const int k_lo = max(kz - 1, 0), k_hi = min(kz + 2, nz);   // own 3-cell window in cbt rows
         float ax = 0.f, ay = 0.f, az = 0.f, dr = 0.f;
         uint32_t sp = stk_base;                                     // shared address of the stack top
@@ -244,7 +256,7 @@ interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict
                     mj = vj.w < 0.f ? ph.mass_bound : ph.mass_fluid;
                     vj.w = fabsf(vj.w);
                 }
-                pair_term<KERNEL>(dx, dy, dz, r2, vi.x, vi.y, vi.z, vi.w, pi.w, ci, vj, pj.w, mj, ph, ax, ay, az, dr);
+                pair_term<KERNEL, GAMMA7>(dx, dy, dz, r2, vi.x, vi.y, vi.z, vi.w, pi.w, ci, vj, pj.w, mj, ph, ax, ay, az, dr);
             }
         };
 
@@ -335,10 +347,10 @@ interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict
     }
 }
 
-template <int KERNEL, bool UNIFORM>
+template <int KERNEL, bool UNIFORM, bool GAMMA7>
 static cudaError_t launch_staged(sph_ctx *c)
 {
-    auto kern = interact_staged_kernel<KERNEL, UNIFORM>;
+    auto kern = interact_staged_kernel<KERNEL, UNIFORM, GAMMA7>;
     static bool attr_set = false;
     if (!attr_set) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(IaSmem));
@@ -399,25 +411,32 @@ cudaError_t launch_pair_stats(sph_ctx *c, unsigned long long *d_out)
     return cudaGetLastError();
 }
 
-cudaError_t launch_interact(sph_ctx *c)
+template <int KERNEL, bool GAMMA7>
+static cudaError_t launch_simple(sph_ctx *c)
 {
     uint32_t n = (uint32_t)c->n;
-    if (n == 0) return cudaSuccess;
-    const bool uni = c->phys.uniform_mass != 0;
-    if (c->interact_variant == 1) {
-        if (c->phys.kernel == 0)
-            interact_simple_kernel<0><<<(n + 127) / 128, 128, 0, c->stream>>>(
-                n, c->pos4[c->cur], c->velrho4[c->cur], c->idt[c->cur], c->keyword, c->cell_begin, c->acc4,
-                c->grid, c->phys);
-        else
-            interact_simple_kernel<1><<<(n + 127) / 128, 128, 0, c->stream>>>(
-                n, c->pos4[c->cur], c->velrho4[c->cur], c->idt[c->cur], c->keyword, c->cell_begin, c->acc4,
-                c->grid, c->phys);
-        c->n_launches++;
+    interact_simple_kernel<KERNEL, GAMMA7><<<(n + 127) / 128, 128, 0, c->stream>>>(
+        n, c->pos4[c->cur], c->velrho4[c->cur], c->idt[c->cur], c->keyword, c->cell_begin, c->acc4, c->grid,
+        c->phys);
+    c->n_launches++;
     return cudaGetLastError();
+}
+
+cudaError_t launch_interact(sph_ctx *c)
+{
+    if (c->n == 0) return cudaSuccess;
+    const bool uni = c->phys.uniform_mass != 0, g7 = c->phys.gamma == 7;
+    const int k = c->phys.kernel;
+    if (c->interact_variant == 1) {
+        if (k == 0) return g7 ? launch_simple<0, true>(c) : launch_simple<0, false>(c);
+        return g7 ? launch_simple<1, true>(c) : launch_simple<1, false>(c);
     }
-    if (c->phys.kernel == 0) return uni ? launch_staged<0, true>(c) : launch_staged<0, false>(c);
-    return uni ? launch_staged<1, true>(c) : launch_staged<1, false>(c);
+    if (k == 0) {
+        if (uni) return g7 ? launch_staged<0, true, true>(c) : launch_staged<0, true, false>(c);
+        return g7 ? launch_staged<0, false, true>(c) : launch_staged<0, false, false>(c);
+    }
+    if (uni) return g7 ? launch_staged<1, true, true>(c) : launch_staged<1, true, false>(c);
+    return g7 ? launch_staged<1, false, true>(c) : launch_staged<1, false, false>(c);
 }
 
 }  // namespace sph
