@@ -132,16 +132,17 @@ interact_simple_kernel(uint32_t n, const float4 *__restrict__ pos4, const float4
 
 // ---- staged production kernel --------------------------------------------------------------------
 constexpr int IA_THREADS = 256;
-constexpr int IA_QCAP = 24;          // stack entries per thread; one entry = 16 candidates' hit mask
-constexpr int IA_SUB = 16;           // candidates tested per stack entry
+constexpr int IA_QCAP = 16;          // stack entries per thread; one entry = hit mask of IA_SUB candidates
+constexpr int IA_SUB = 20;           // candidates tested per stack entry (entry = index << 20 | 20-bit mask)
 constexpr int IA_ZMAX = 32;          // max cells per z-block
-constexpr int IA_CAP = 2688;         // staged candidates per batch (9 columns x 11 cells x 27 + slack)
+constexpr int IA_CAP = 2688;         // staged candidates per batch (9 columns x 11 cells x 27 + slack), < 4096
 constexpr float IA_TINY = 1e-30f;    // r2 floor: a coincident pair (the particle itself) adds exactly 0
 
 struct IaSmem {
-    float4 pos[IA_CAP];                       // x, y, z, p/rho^2
+    float4 rel[IA_CAP];                       // position relative to the CTA origin, and its square norm
     float4 vr[IA_CAP];                        // vx, vy, vz, rho (sign bit = boundary type if masses differ)
-    uint32_t stack[IA_QCAP * IA_THREADS];     // [entry][thread]: byte offset of 16 candidates << 16 | hit mask
+    float pr[IA_CAP];                         // p/rho^2
+    uint32_t stack[IA_QCAP * IA_THREADS];     // [entry][thread]: first candidate index << 20 | hit mask
     uint32_t cbt[9][IA_ZMAX + 3];             // cell_begin of the 9 columns over [zlo, zhi]
     uint32_t col_vstart[10];                  // virtual start of each column in the concatenation
     uint32_t stage_lo[9], stage_hi[9];        // global index range of the column staged in this batch
@@ -160,11 +161,28 @@ __device__ __forceinline__ uint32_t lds_u32(uint32_t addr)
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
     return v;
 }
+__device__ __forceinline__ float lds_f32(uint32_t addr)
+{
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
+    return v;
+}
 __device__ __forceinline__ float4 lds_f4(uint32_t addr)
 {
     float4 v;
     asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
     return v;
+}
+
+// Origin of the CTA-relative coordinates along one axis.  x - O is EXACT in fp32 for every staged
+// particle (so relative differences equal absolute differences bit for bit): O = 0 when the CTA's
+// neighbourhood (reach D around `corner`) is within 2D of the coordinate plane, else `corner` with
+// its two lowest mantissa bits cleared, which makes O a multiple of ulp(x) for all |x| <= |O| + D
+// while |x - O| <= D <= |x| keeps the difference inside 24 bits.
+__device__ __forceinline__ float rel_origin(float corner, float reach)
+{
+    if (fabsf(corner) < 2.0f * reach) return 0.0f;
+    return __uint_as_float(__float_as_uint(corner) & ~3u);
 }
 
 template <int KERNEL, bool UNIFORM, bool GAMMA7>
@@ -200,6 +218,11 @@ interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict
             v = cell_begin[(uint32_t)(x * g.nc[1] + y) * g.nc[2] + zlo + z];
         S.cbt[col][z] = v;          // columns outside the grid: all 0 => empty ranges
     }
+    // ---- CTA-relative coordinate origin (same value in every thread)
+    const float cell = 2.0f * ph.h;
+    const float ox = rel_origin(fmaf((float)cx, cell, g.min[0]), 4.0f * cell);
+    const float oy = rel_origin(fmaf((float)cy, cell, g.min[1]), 4.0f * cell);
+    const float oz = rel_origin(fmaf((float)cz0, cell, g.min[2]), (float)(zb + 3) * cell);
     __syncthreads();
     if (tid == 0) {
         uint32_t acc = 0;
@@ -212,16 +235,19 @@ interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict
     __syncthreads();
     const uint32_t total = S.col_vstart[9];
     const uint32_t lane_full = 0xffffffffu;
-    const uint32_t pos_base = (uint32_t)__cvta_generic_to_shared(S.pos);
-    const uint32_t vr_delta = (uint32_t)__cvta_generic_to_shared(S.vr) - pos_base;
+    const uint32_t rel_base = (uint32_t)__cvta_generic_to_shared(S.rel);
+    const uint32_t vr_delta = (uint32_t)__cvta_generic_to_shared(S.vr) - rel_base;
+    const uint32_t pr_base = (uint32_t)__cvta_generic_to_shared(S.pr);
     const uint32_t stk_base = (uint32_t)__cvta_generic_to_shared(S.stack) + 4u * tid;
     constexpr uint32_t STK_STRIDE = 4u * IA_THREADS;
-    const uint32_t stk_high = stk_base + STK_STRIDE * (IA_QCAP - 2);
+    const uint32_t stk_high = stk_base + STK_STRIDE * (IA_QCAP - 1);   // sp above this = stack full
+    // conservative filter radius: rounding of the expanded form is < 3e-3 h^2
+    const float filt2 = ph.four_h2 + 0.02f * ph.h * ph.h;
 
     for (uint32_t chunk = t_begin; chunk < t_end; chunk += IA_THREADS) {
         const uint32_t i = chunk + tid;
         const bool active = i < t_end;
-        float4 pi = make_float4(0.f, 0.f, 0.f, 0.f), vi = make_float4(0.f, 0.f, 0.f, 1.f);
+        float4 pi = make_float4(ox, oy, oz, 0.f), vi = make_float4(0.f, 0.f, 0.f, 1.f);
         int kz = 0;
         bool fluid = false;
         if (active) {
@@ -230,34 +256,52 @@ interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict
             fluid = (idt[i] & TYPE_BIT) == 0;
             kz = (int)((keyword[i] & CELL_MASK) - own_col) - zlo;   // own cz - zlo
         }
+        const float xi = pi.x - ox, yi = pi.y - oy, zi = pi.z - oz;  // exact
+        const float fa = -2.0f * xi, fb = -2.0f * yi, fc = -2.0f * zi;
+        const float fT = filt2 - fmaf(zi, zi, fmaf(yi, yi, xi * xi));
         const float ci = sound_speed<GAMMA7>(vi.w, ph);
         const int k_lo = max(kz - 1, 0), k_hi = min(kz + 2, nz);   // own 3-cell window in cbt rows
         float ax = 0.f, ay = 0.f, az = 0.f, dr = 0.f;
         uint32_t sp = stk_base;                                     // shared address of the stack top
+        uint32_t cur_mask = 0, cur_s = 0;                           // entry being drained
 
-        uint32_t cur_mask = 0, cur_o = 0;                          // entry being drained
-        auto drain_one = [&]() {
+        // next pending candidate of this lane: smem index s, or ok = false
+        auto pop = [&](uint32_t &s, bool &ok) {
             if (cur_mask == 0 && sp > stk_base) {
                 sp -= STK_STRIDE;
                 const uint32_t e = lds_u32(sp);
-                cur_mask = e & 0xFFFFu;
-                cur_o = e >> 16;
+                cur_mask = e & 0xFFFFFu;
+                cur_s = e >> 20;
             }
-            if (cur_mask) {
-                const uint32_t bit = __ffs(cur_mask) - 1;
-                cur_mask &= cur_mask - 1;
-                const uint32_t o = cur_o + 16u * bit;
-                const float4 pj = lds_f4(pos_base + o);
-                float4 vj = lds_f4(pos_base + vr_delta + o);
-                const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
-                const float r2 = fmaxf(fmaf(dz, dz, fmaf(dy, dy, dx * dx)), IA_TINY);
-                float mj = 1.0f;
-                if (!UNIFORM) {
-                    mj = vj.w < 0.f ? ph.mass_bound : ph.mass_fluid;
-                    vj.w = fabsf(vj.w);
-                }
-                pair_term<KERNEL, GAMMA7>(dx, dy, dz, r2, vi.x, vi.y, vi.z, vi.w, pi.w, ci, vj, pj.w, mj, ph, ax, ay, az, dr);
+            ok = cur_mask != 0;
+            s = cur_s + (uint32_t)(__ffs(cur_mask) - 1);
+            cur_mask &= cur_mask - 1;
+        };
+        // pair term of candidate s; ok = false turns it into a no-op without a branch (s = 0 is
+        // always a staged, finite candidate; its mass factor is zeroed)
+        auto interact = [&](uint32_t s, bool ok) {
+            s = ok ? s : 0u;
+            const float4 rj = lds_f4(rel_base + 16u * s);
+            float4 vj = lds_f4(rel_base + vr_delta + 16u * s);
+            const float Pj = lds_f32(pr_base + 4u * s);
+            const float dx = xi - rj.x, dy = yi - rj.y, dz = zi - rj.z;     // == absolute differences
+            const float r2 = fmaxf(fmaf(dz, dz, fmaf(dy, dy, dx * dx)), IA_TINY);
+            float mj = ok ? 1.0f : 0.0f;
+            if (!UNIFORM) {
+                mj = ok ? (vj.w < 0.f ? ph.mass_bound : ph.mass_fluid) : 0.0f;
+                vj.w = fabsf(vj.w);
             }
+            pair_term<KERNEL, GAMMA7>(dx, dy, dz, r2, vi.x, vi.y, vi.z, vi.w, pi.w, ci, vj, Pj, mj, ph,
+                                      ax, ay, az, dr);
+        };
+        // one drain round: up to two pending pairs per lane, as two interleaved dependency chains
+        auto drain_round = [&]() {
+            uint32_t s0, s1;
+            bool ok0, ok1;
+            pop(s0, ok0);
+            pop(s1, ok1);
+            interact(s0, ok0);
+            interact(s1, ok1);
         };
 
         for (uint32_t bstart = 0; bstart < total; bstart += IA_CAP) {
@@ -281,10 +325,13 @@ interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict
                 const uint32_t lo = S.stage_lo[col], hi = S.stage_hi[col];
                 const int32_t off = S.stage_off[col];
                 for (uint32_t j = lo + tid; j < hi; j += IA_THREADS) {
-                    S.pos[(int32_t)j + off] = __ldg(pos4 + j);
+                    const float4 p = __ldg(pos4 + j);
                     float4 v = __ldg(velrho4 + j);
                     if (!UNIFORM && (__ldg(idt + j) & TYPE_BIT)) v.w = -v.w;
+                    const float xr = p.x - ox, yr = p.y - oy, zr = p.z - oz;
+                    S.rel[(int32_t)j + off] = make_float4(xr, yr, zr, fmaf(zr, zr, fmaf(yr, yr, xr * xr)));
                     S.vr[(int32_t)j + off] = v;
+                    S.pr[(int32_t)j + off] = p.w;
                 }
             }
             __syncthreads();
@@ -299,44 +346,44 @@ interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict
                 const int off = S.stage_off[col];
                 const int len = max(hi - lo, 0);
                 const int maxlen = __reduce_max_sync(lane_full, len);
-                // lanes without work in this column read from offset 0 and record nothing
+                // lanes without work in this column read from index 0 and record nothing
                 const bool work = len > 0;
                 const int minlen = __reduce_min_sync(lane_full, work ? len : 0x7fffffff);
-                // byte offsets into pos[]: candidate t of this lane is at o + 16 t, valid while < o_hi
-                uint32_t o = work ? (uint32_t)(lo + off) * 16u : 0u;
-                const uint32_t o_hi = o + (uint32_t)len * 16u;
+                uint32_t s = work ? (uint32_t)(lo + off) : 0u;       // smem index of the next candidate
+                const uint32_t s_hi = s + (uint32_t)len;
                 int sb = 0;
-                // sub-batches of 16 that are complete for every working lane: no range checks
-                for (; sb + IA_SUB <= minlen && sb < maxlen; sb += IA_SUB, o += 16u * IA_SUB) {
+                // sub-batches of IA_SUB that are complete for every working lane: no range checks.
+                // |r_ij|^2 < R^2  <=>  |r_j|^2 - 2 r_i.r_j < R^2 - |r_i|^2   (3 FFMA + 1 compare)
+                for (; sb + IA_SUB <= minlen && sb < maxlen; sb += IA_SUB, s += IA_SUB) {
                     uint32_t mask = 0;
+                    const uint32_t a0 = rel_base + 16u * s;
 #pragma unroll
                     for (int u = 0; u < IA_SUB; ++u) {
-                        const float4 pj = lds_f4(pos_base + o + 16u * u);
-                        const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
-                        const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                        if (r2 < ph.four_h2) mask |= 1u << u;
+                        const float4 rj = lds_f4(a0 + 16u * u);
+                        if (fmaf(fc, rj.z, fmaf(fb, rj.y, fmaf(fa, rj.x, rj.w))) < fT) mask |= 1u << u;
                     }
-                    if (work && mask) { sts_u32(sp, (o << 16) | mask); sp += STK_STRIDE; }
-                    while (__any_sync(lane_full, sp > stk_high)) drain_one();
+                    if (work && mask) { sts_u32(sp, (s << 20) | mask); sp += STK_STRIDE; }
+                    while (__any_sync(lane_full, sp > stk_high)) drain_round();
                 }
-                // ragged remainder in groups of 4 with per-lane range checks (reads past o_hi stay
-                // inside the CTA's shared memory: o < 16 IA_CAP and advances by at most 16 IA_CAP)
-                for (; sb < maxlen; sb += 4, o += 64u) {
+                // ragged remainder in groups of 4 with per-lane range checks (reads past s_hi stay
+                // inside the CTA's shared memory: s < IA_CAP and advances by at most IA_CAP)
+                for (; sb < maxlen; sb += 4, s += 4) {
                     uint32_t mask = 0;
+                    const uint32_t a0 = rel_base + 16u * s;
 #pragma unroll
                     for (int u = 0; u < 4; ++u) {
-                        const uint32_t ou = o + 16u * u;
-                        const float4 pj = lds_f4(pos_base + ou);
-                        const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
-                        const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                        if (ou < o_hi && r2 < ph.four_h2) mask |= 1u << u;
+                        const float4 rj = lds_f4(a0 + 16u * u);
+                        if (s + u < s_hi && fmaf(fc, rj.z, fmaf(fb, rj.y, fmaf(fa, rj.x, rj.w))) < fT) mask |= 1u << u;
                     }
-                    if (mask) { sts_u32(sp, (o << 16) | mask); sp += STK_STRIDE; }
-                    while (__any_sync(lane_full, sp > stk_high)) drain_one();
+                    if (mask) { sts_u32(sp, (s << 20) | mask); sp += STK_STRIDE; }
+                    while (__any_sync(lane_full, sp > stk_high)) drain_round();
                 }
+                // drain completely after every third column (and before the staged data is replaced):
+                // all lanes then hold ~40 pending pairs, so nearly every lane works in every round;
+                // the capacity-triggered drains above are only a safety net for dense cells
+                if (col % 3 == 2)
+                    while (__any_sync(lane_full, (sp > stk_base) || cur_mask != 0)) drain_round();
             }
-            // ---- flush the stacks before the staged data is replaced
-            while (__any_sync(lane_full, (sp > stk_base) || cur_mask != 0)) drain_one();
         }
         if (active) {
             if (UNIFORM) { ax *= ph.mass_fluid; ay *= ph.mass_fluid; az *= ph.mass_fluid; dr *= ph.mass_fluid; }
