@@ -132,7 +132,7 @@ interact_simple_kernel(uint32_t n, const float4 *__restrict__ pos4, const float4
 
 // ---- staged production kernel --------------------------------------------------------------------
 constexpr int IA_THREADS = 256;
-constexpr int IA_QCAP = 16;          // stack entries per thread; one entry = hit mask of IA_SUB candidates
+constexpr int IA_QCAP = 17;          // stack entries per thread; one entry = hit mask of IA_SUB candidates
 constexpr int IA_SUB = 20;           // candidates tested per stack entry (entry = index << 20 | 20-bit mask)
 constexpr int IA_ZMAX = 32;          // max cells per z-block
 constexpr int IA_CAP = 2688;         // staged candidates per batch (9 columns x 11 cells x 27 + slack), < 4096
@@ -378,12 +378,11 @@ interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict
                     if (mask) { sts_u32(sp, (s << 20) | mask); sp += STK_STRIDE; }
                     while (__any_sync(lane_full, sp > stk_high)) drain_round();
                 }
-                // drain completely after every third column (and before the staged data is replaced):
-                // all lanes then hold ~40 pending pairs, so nearly every lane works in every round;
-                // the capacity-triggered drains above are only a safety net for dense cells
-                if (col % 3 == 2)
-                    while (__any_sync(lane_full, (sp > stk_base) || cur_mask != 0)) drain_round();
             }
+            // ---- flush the stacks before the staged data is replaced.  Until here the stacks are
+            // kept as full as they can be (drains only when some lane's stack is full), so that
+            // nearly every lane has a pending pair in every drain round.
+            while (__any_sync(lane_full, (sp > stk_base) || cur_mask != 0)) drain_round();
         }
         if (active) {
             if (UNIFORM) { ax *= ph.mass_fluid; ay *= ph.mass_fluid; az *= ph.mass_fluid; dr *= ph.mass_fluid; }
