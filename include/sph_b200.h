@@ -23,7 +23,7 @@
  *     sph_profile_read and sph_init/sph_set_state with HOST inputs, which synchronise it.
  *   - Return value: SPH_OK (0) or a negative SPH_ERR_* code; no exceptions, no abort, no
  *     CPU fallback.  sph_strerror() names a code.
- *   - Particle k of the input has id k.  n < 2^28; number of grid cells <= 2^28.
+ *   - Particle k of the input has id k.  n <= 2^28; number of grid cells <= 2^28.
  *   - Precision: fp32 state and arithmetic (the paper does not state its precision, L35).
  */
 #ifndef SPH_B200_H
@@ -42,7 +42,7 @@ enum {
     SPH_OK = 0,
     SPH_ERR_ARG = -1,             /* NULL / out-of-range argument */
     SPH_ERR_WORKSPACE = -2,       /* workspace NULL, misaligned or too small */
-    SPH_ERR_GRID_TOO_LARGE = -3,  /* more than 2^28 cells, or n >= 2^28 */
+    SPH_ERR_GRID_TOO_LARGE = -3,  /* more than 2^28 cells, or n > 2^28 */
     SPH_ERR_SLABS = -4,           /* planes not 0 = p0 < p1 < ... < pS = ncx, a slab thinner
                                      than 2 cell planes (S > 1), or S > max_slabs */
     SPH_ERR_CUDA = -5,            /* a CUDA runtime call failed (sticky) */

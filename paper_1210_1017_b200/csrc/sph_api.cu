@@ -42,7 +42,7 @@ bool make_layout(const sph_params *p, uint64_t n, int max_slabs, Layout *L)
 {
     int nc[3];
     uint64_t ncells;
-    if (!p || n >= (1ull << 28) || max_slabs < 1 || max_slabs > SPH_MAX_SLABS) return false;
+    if (!p || n > (1ull << 28) || max_slabs < 1 || max_slabs > SPH_MAX_SLABS) return false;
     if (!grid_of(p, nc, &ncells)) return false;
     size_t off = 0;
     size_t nn = n ? n : 1;
@@ -223,7 +223,7 @@ int sph_init(sph_ctx **out, const sph_params *p, const sph_particles *part, int 
         return SPH_ERR_ARG;
     int nc[3];
     uint64_t ncells;
-    if (part->n >= (1ull << 28)) return SPH_ERR_GRID_TOO_LARGE;
+    if (part->n > (1ull << 28)) return SPH_ERR_GRID_TOO_LARGE;
     if (!grid_of(p, nc, &ncells)) {
         for (int k = 0; k < 3; ++k)
             if (!(p->dom_max[k] > p->dom_min[k])) return SPH_ERR_ARG;
@@ -555,7 +555,7 @@ const char *sph_strerror(int code)
     case SPH_OK: return "ok";
     case SPH_ERR_ARG: return "bad argument";
     case SPH_ERR_WORKSPACE: return "workspace missing, misaligned or too small";
-    case SPH_ERR_GRID_TOO_LARGE: return "grid has more than 2^28 cells or n >= 2^28";
+    case SPH_ERR_GRID_TOO_LARGE: return "grid has more than 2^28 cells or n > 2^28";
     case SPH_ERR_SLABS: return "bad slab planes";
     case SPH_ERR_CUDA: return "CUDA runtime error";
     case SPH_ERR_NONFINITE: return "non-finite particle state on the device";

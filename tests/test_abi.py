@@ -47,7 +47,7 @@ def test_workspace_bytes_and_argument_errors(B):
     b1 = B.sph_workspace_bytes(p, w.n, 1)
     b16 = B.sph_workspace_bytes(p, w.n, 16)
     assert 0 < b1 < b16 < 400 * w.n + (1 << 22)
-    assert B.sph_workspace_bytes(p, 1 << 28, 1) == 0          # n too large
+    assert B.sph_workspace_bytes(p, (1 << 28) + 1, 1) == 0    # n too large
     assert B.sph_workspace_bytes(p, w.n, 17) == 0             # too many slabs
     big = dict(w.params)
     big["dom_max"] = (1e4, 1e4, 1e4)                          # > 2^28 cells
