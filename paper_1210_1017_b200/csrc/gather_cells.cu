@@ -65,17 +65,6 @@ constexpr int CF_IPT = 16;
 constexpr int CF_TILE = CF_THREADS * CF_IPT;
 uint32_t scan_tiles(uint64_t n) { return (uint32_t)((n + CF_TILE - 1) / CF_TILE); }
 
-__device__ __forceinline__ unsigned long long ld_relaxed64(const unsigned long long *p)
-{
-    unsigned long long v;
-    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
-    return v;
-}
-__device__ __forceinline__ void st_relaxed64(unsigned long long *p, unsigned long long v)
-{
-    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
-}
-
 // Tiles are numbered from the END of the array (tile 0 holds the last elements), so that the
 // suffix scan is a forward chained scan over tiles.  state word: flag<<32 | value.
 __global__ void __launch_bounds__(CF_THREADS)
@@ -119,23 +108,15 @@ cell_fill_kernel(uint32_t m /* ncells+1 */, uint32_t n, uint32_t *__restrict__ c
         block_min = min(block_min, t);
     }
     exc = min(exc, wpre);
-    // chained look-back over earlier tiles (= later cells)
-    if (tid == 0) {
-        st_relaxed64(state + tile, ((tile == 0 ? 2ull : 1ull) << 32) | block_min);
+    // chained look-back over earlier tiles (= later cells), warp 0, 32 tiles per round trip
+    if (warp == 0) {
+        if (lane == 0) st_relaxed_u64(state + tile, ((tile == 0 ? 2ull : 1ull) << 32) | block_min);
         uint32_t carry = 0xFFFFFFFFu;
         if (tile > 0) {
-            int t = (int)tile - 1;
-            while (true) {
-                unsigned long long s = ld_relaxed64(state + t);
-                uint32_t f = (uint32_t)(s >> 32);
-                if (f == 0) continue;
-                carry = min(carry, (uint32_t)s);
-                if (f == 2) break;
-                --t;
-            }
-            st_relaxed64(state + tile, (2ull << 32) | min(carry, block_min));
+            carry = warp_lookback(state, tile, 0xFFFFFFFFu, [](uint32_t a, uint32_t b) { return min(a, b); });
+            if (lane == 0) st_relaxed_u64(state + tile, (2ull << 32) | min(carry, block_min));
         }
-        s_carry = carry;
+        if (lane == 0) s_carry = carry;
     }
     __syncthreads();
     exc = min(exc, s_carry);

@@ -51,17 +51,6 @@ constexpr int MG_THREADS = 256;
 constexpr int MG_IPT = 16;
 constexpr int MG_TILE = MG_THREADS * MG_IPT;
 
-__device__ __forceinline__ unsigned long long ld_relaxed64m(const unsigned long long *p)
-{
-    unsigned long long v;
-    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
-    return v;
-}
-__device__ __forceinline__ void st_relaxed64m(unsigned long long *p, unsigned long long v)
-{
-    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
-}
-
 __global__ void __launch_bounds__(MG_THREADS)
 migrants_kernel(uint32_t n, const uint32_t *__restrict__ keyword, const uint2 *__restrict__ kv,
                 const uint32_t *__restrict__ idt, SlabC sl, int nyz, unsigned long long *state,
@@ -96,23 +85,17 @@ migrants_kernel(uint32_t n, const uint32_t *__restrict__ keyword, const uint2 *_
         if (w < (int)warp) wpre += t;
         total += t;
     }
-    if (tid == 0) {
-        st_relaxed64m(state + tile, ((tile == 0 ? 2ull : 1ull) << 32) | total);
+    if (warp == 0) {                     // look-back by warp 0, 32 tiles per round trip
+        if (lane == 0) st_relaxed_u64(state + tile, ((tile == 0 ? 2ull : 1ull) << 32) | total);
         uint32_t carry = 0;
         if (tile > 0) {
-            int t = (int)tile - 1;
-            while (true) {
-                unsigned long long s = ld_relaxed64m(state + t);
-                uint32_t f = (uint32_t)(s >> 32);
-                if (f == 0) continue;
-                carry += (uint32_t)s;
-                if (f == 2) break;
-                --t;
-            }
-            st_relaxed64m(state + tile, (2ull << 32) | (carry + total));
+            carry = warp_lookback(state, tile, 0u, [](uint32_t a, uint32_t b) { return a + b; });
+            if (lane == 0) st_relaxed_u64(state + tile, (2ull << 32) | (carry + total));
         }
-        s_carry = carry;
-        if (tile == gridDim.x - 1) *mig_total = carry + total;   // tiles are ticketed in order
+        if (lane == 0) {
+            s_carry = carry;
+            if (tile == gridDim.x - 1) *mig_total = carry + total;   // tiles are ticketed in order
+        }
     }
     __syncthreads();
     uint32_t out = s_carry + wpre + inc - cnt;

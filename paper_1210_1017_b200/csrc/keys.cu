@@ -54,25 +54,22 @@ __device__ __forceinline__ int cell_coord(float x, float mn, float inv, int nc)
     return min(max(ci, 0), nc - 1);
 }
 
-__device__ __forceinline__ int slab_of_plane(int cx, const SlabC &s)
+// Largest s with table[s] <= x, for a shared-memory table of 17 ascending entries padded with
+// "infinity" beyond the used ones (4 probes instead of a 15-way compare chain).
+template <typename T>
+__device__ __forceinline__ int upper_slot(const T *table, T x)
 {
-    int k = 0;
+    int s = 0;
 #pragma unroll
-    for (int j = 1; j < SPH_MAX_SLABS; ++j)
-        k += (j < s.n_slabs && cx >= s.planes[j]) ? 1 : 0;
-    return k;
-}
-
-__device__ __forceinline__ uint32_t edge_label(int cx, int slab, const SlabC &s)
-{
-    uint32_t lab = 0;
-    if (slab > 0 && cx == s.planes[slab]) lab = 1;
-    if (slab < s.n_slabs - 1 && cx == s.planes[slab + 1] - 1) lab = 2;
-    return lab;
+    for (int step = 8; step >= 1; step >>= 1)
+        s += (x >= table[s + step]) ? step : 0;
+    return s;
 }
 
 // prev_mode: 0 = none (no migrants), 1 = previous slab ranges over the current order,
 //            2 = caller-supplied prev_init[id]
+constexpr int KEYS_IPT = 4;          // particles per thread per iteration (independent loads in flight)
+
 template <int PASSES>
 __global__ void __launch_bounds__(256)
 keys_kernel(uint32_t n, const float4 *__restrict__ pos4, const uint32_t *__restrict__ idt,
@@ -82,46 +79,68 @@ keys_kernel(uint32_t n, const float4 *__restrict__ pos4, const uint32_t *__restr
 {
     __shared__ uint32_t s_hist[PASSES * 256];
     __shared__ uint32_t s_prev_begin[SPH_MAX_SLABS + 1];
+    __shared__ int s_planes[SPH_MAX_SLABS + 2];
     for (int k = threadIdx.x; k < PASSES * 256; k += blockDim.x) s_hist[k] = 0;
-    if (prev_mode == 1 && threadIdx.x <= prev_n) s_prev_begin[threadIdx.x] = prev_slab_begin[threadIdx.x];
+    if (threadIdx.x <= SPH_MAX_SLABS) {
+        const int t = threadIdx.x;
+        s_planes[t] = t < sl.n_slabs ? sl.planes[t] : 0x7fffffff;          // planes[S] = ncx is never reached
+        s_prev_begin[t] = (prev_mode == 1 && t < prev_n) ? prev_slab_begin[t] : 0xffffffffu;
+        if (t == 0) { s_planes[SPH_MAX_SLABS + 1] = 0x7fffffff; s_prev_begin[0] = 0; }
+    }
     __syncthreads();
 
-    const uint32_t lane = threadIdx.x & 31;
+    const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const uint32_t lt_mask = (1u << lane) - 1u;
-    const uint32_t stride = gridDim.x * blockDim.x;
-    const uint32_t n_round = (n + 31u) & ~31u;    // keep warps converged for match_any
-    for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n_round; i += stride) {
-        bool valid = i < n;
-        uint32_t cell = 0;
-        if (valid) {
-            float4 p = pos4[i];
-            uint32_t w = idt[i];
-            uint32_t id = w & ID_MASK;
-            if (!(isfinite(p.x) && isfinite(p.y) && isfinite(p.z))) atomicOr(flags, FLAG_NONFINITE);
-            int cx = cell_coord(p.x, g.min[0], g.inv_cell, g.nc[0]);
-            int cy = cell_coord(p.y, g.min[1], g.inv_cell, g.nc[1]);
-            int cz = cell_coord(p.z, g.min[2], g.inv_cell, g.nc[2]);
-            cell = (uint32_t)((cx * g.nc[1] + cy) * g.nc[2] + cz);
-            int slab = slab_of_plane(cx, sl);
-            int prev = slab;
-            if (prev_mode == 1) {
-                prev = 0;
+    const int S = sl.n_slabs;
+    constexpr uint32_t WCHUNK = 32 * KEYS_IPT;
+    const uint32_t stride = gridDim.x * (blockDim.x >> 5) * WCHUNK;
+    // a warp owns WCHUNK consecutive particles per iteration; the loop bound is warp-uniform, so
+    // the warp stays converged for match_any
+    for (uint32_t base = (blockIdx.x * (blockDim.x >> 5) + warp) * WCHUNK; base < n; base += stride) {
+        float4 p[KEYS_IPT];
+        uint32_t w[KEYS_IPT];
 #pragma unroll
-                for (int j = 1; j < SPH_MAX_SLABS; ++j)
-                    prev += (j < prev_n && i >= s_prev_begin[j]) ? 1 : 0;
-            } else if (prev_mode == 2) {
-                prev = min((int)prev_init[id], sl.n_slabs - 1);
-            }
-            uint32_t mig = slab < prev ? 1u : (slab > prev ? 2u : 0u);
-            uint32_t tag = edge_label(cx, slab, sl) | (mig << 2);
-            kv_by_id[id] = make_uint2((tag << TAG_SHIFT) | cell, ((uint32_t)prev << 28) | i);
+        for (int k = 0; k < KEYS_IPT; ++k) {
+            const uint32_t i = base + k * 32 + lane;
+            if (i < n) { p[k] = __ldg(pos4 + i); w[k] = __ldg(idt + i); }
+            else { p[k] = make_float4(0.f, 0.f, 0.f, 0.f); w[k] = 0; }
         }
-        // warp-aggregated digit histograms (one shared-memory atomic per distinct digit)
 #pragma unroll
-        for (int p = 0; p < PASSES; ++p) {
-            uint32_t d = valid ? ((cell >> (8 * p)) & 255u) : (256u + lane);
-            uint32_t m = __match_any_sync(0xffffffffu, d);
-            if (valid && (m & lt_mask) == 0) atomicAdd(&s_hist[p * 256 + d], __popc(m));
+        for (int k = 0; k < KEYS_IPT; ++k) {
+            const uint32_t i = base + k * 32 + lane;
+            const bool valid = i < n;
+            uint32_t cell = 0;
+            if (valid) {
+                const uint32_t id = w[k] & ID_MASK;
+                if (!(isfinite(p[k].x) && isfinite(p[k].y) && isfinite(p[k].z))) atomicOr(flags, FLAG_NONFINITE);
+                const int cx = cell_coord(p[k].x, g.min[0], g.inv_cell, g.nc[0]);
+                const int cy = cell_coord(p[k].y, g.min[1], g.inv_cell, g.nc[1]);
+                const int cz = cell_coord(p[k].z, g.min[2], g.inv_cell, g.nc[2]);
+                cell = (uint32_t)((cx * g.nc[1] + cy) * g.nc[2] + cz);
+                const int slab = upper_slot(s_planes, cx);
+                uint32_t lab = 0;                                          // edge label (L240)
+                if (slab > 0 && cx == s_planes[slab]) lab = 1;
+                if (slab < S - 1 && cx == s_planes[slab + 1] - 1) lab = 2;
+                int prev = slab;
+                if (prev_mode == 1) prev = upper_slot(s_prev_begin, i);
+                else if (prev_mode == 2) prev = min((int)prev_init[id], S - 1);
+                const uint32_t mig = slab < prev ? 1u : (slab > prev ? 2u : 0u);   // migration label (L264)
+                const uint32_t tag = lab | (mig << 2);
+                kv_by_id[id] = make_uint2((tag << TAG_SHIFT) | cell, ((uint32_t)prev << 28) | i);
+            }
+            // warp-aggregated digit histograms (one shared-memory atomic per distinct digit)
+#pragma unroll
+            for (int q = 0; q < PASSES; ++q) {
+                const uint32_t d = (cell >> (8 * q)) & 255u;
+                const uint32_t d0 = __shfl_sync(0xffffffffu, d, 0);
+                const uint32_t vmask = __ballot_sync(0xffffffffu, valid);
+                if (__all_sync(0xffffffffu, !valid || d == d0)) {           // one digit in the whole warp
+                    if (lane == 0 && vmask) atomicAdd(&s_hist[q * 256 + d0], __popc(vmask));
+                } else {
+                    const uint32_t m = warp_match8(d, valid);
+                    if (valid && (m & lt_mask) == 0) atomicAdd(&s_hist[q * 256 + d], __popc(m));
+                }
+            }
         }
     }
     __syncthreads();
@@ -138,7 +157,7 @@ cudaError_t launch_keys(sph_ctx *c)
     if (e != cudaSuccess) return e;
     if (n == 0) return cudaSuccess;
     int prev_mode = c->have_prev_init ? 2 : (c->have_prev_ranges ? 1 : 0);
-    uint32_t blocks = (n + 255) / 256;
+    uint32_t blocks = (n + 256 * KEYS_IPT - 1) / (256 * KEYS_IPT);
     uint32_t cap = NUM_SMS * 8;
     if (blocks > cap) blocks = cap;
     const float4 *pos4 = c->pos4[c->cur];

@@ -6,7 +6,7 @@
 //
 // One kernel per 8-bit digit.  The digit histograms come from the key kernel (keys.cu); each
 // pass is a single sweep: a CTA takes a tile in launch order (dynamic tile id), ranks its keys
-// with warp-level match_any + per-warp shared-memory counters (stable), publishes its 256 digit
+// with a warp-level match (ballots) + per-warp shared-memory counters (stable), publishes its 256 digit
 // counts, resolves the exclusive prefix over earlier tiles by decoupled look-back, reorders the
 // tile through shared memory and writes runs of equal digits to consecutive addresses.
 //
@@ -19,6 +19,7 @@ constexpr int RS_THREADS = 512;
 constexpr int RS_IPT = 12;                        // pairs per thread
 constexpr int RS_TILE = RS_THREADS * RS_IPT;      // 6144 pairs = 48 KB staged
 constexpr int RS_WARPS = RS_THREADS / 32;
+constexpr int RS_LB = 8;                          // look-back polls in flight per thread
 constexpr uint32_t LB_AGG = 1u << 30;             // look-back word: flag in bits 30..31
 constexpr uint32_t LB_INC = 2u << 30;
 constexpr uint32_t LB_VAL = (1u << 30) - 1u;
@@ -45,7 +46,7 @@ struct __align__(16) RsSmem {
     uint32_t tile;
 };
 
-__global__ void __launch_bounds__(RS_THREADS)
+__global__ void __launch_bounds__(RS_THREADS, 2)
 onesweep_kernel(uint32_t n, const uint2 *__restrict__ in, uint2 *__restrict__ out,
                 const uint32_t *__restrict__ hist, uint32_t *tile_state, uint32_t *tile_counter, int shift,
                 uint32_t dmask /* keeps the tag bits 28..31 out of the last digit */)
@@ -64,7 +65,7 @@ onesweep_kernel(uint32_t n, const uint2 *__restrict__ in, uint2 *__restrict__ ou
 
     // ---- load, warp-striped: the warp owns a contiguous chunk; item k of lane l is chunk[k*32+l]
     uint2 kv[RS_IPT];
-    uint32_t rank[RS_IPT];
+    uint32_t rank2[RS_IPT / 2];                   // warp-local ranks, two 16-bit values per word
     const uint32_t wbase = warp * (32 * RS_IPT);
 #pragma unroll
     for (int k = 0; k < RS_IPT; ++k) {
@@ -77,29 +78,35 @@ onesweep_kernel(uint32_t n, const uint2 *__restrict__ in, uint2 *__restrict__ ou
     for (int k = 0; k < RS_IPT; ++k) {
         uint32_t li = wbase + k * 32 + lane;
         bool valid = li < tile_n;
-        uint32_t d = valid ? ((kv[k].x >> shift) & dmask) : (256u + lane);
-        uint32_t m = __match_any_sync(0xffffffffu, d);
+        uint32_t d = (kv[k].x >> shift) & dmask;
+        uint32_t m = warp_match8(d, valid);
         uint32_t leader = __ffs(m) - 1;
         uint32_t old = 0;
         if (valid && lane == leader) { old = wh[d]; wh[d] = old + __popc(m); }
         old = __shfl_sync(0xffffffffu, old, leader);
-        rank[k] = old + __popc(m & lt_mask);
+        const uint32_t r = old + __popc(m & lt_mask);
+        if (k & 1) rank2[k >> 1] |= r << 16; else rank2[k >> 1] = r;
         __syncwarp();
     }
     __syncthreads();
 
-    // ---- per digit (threads 0..255): scan over warps, publish, look back
-    uint32_t exc_in_warp = 0, hexc_in_warp = 0, lookback = 0;
+    // ---- per digit (threads 0..255): counts over warps, publish the tile aggregate at once, and
+    // put the first round of look-back polls in flight; their latency (and the predecessors'
+    // progress) overlaps the local scan and the shared-memory reordering below
+    uint32_t count = 0, exc_in_warp = 0, hexc_in_warp = 0;
+    uint32_t poll[RS_LB];
+    uint32_t *st = tile_state + (size_t)tile * 256 + (tid & 255);
     if (tid < 256) {
-        uint32_t count = 0;
 #pragma unroll
         for (int w = 0; w < RS_WARPS; ++w) {
             uint32_t t = S.warp_hist[w][tid];
             S.warp_hist[w][tid] = count;
             count += t;
         }
-        uint32_t *st = tile_state + (size_t)tile * 256 + tid;
-        st_relaxed(st, (tile == 0 ? LB_INC : LB_AGG) | count);     // publish first
+        st_relaxed(st, (tile == 0 ? LB_INC : LB_AGG) | count);
+#pragma unroll
+        for (int b = 0; b < RS_LB; ++b)
+            poll[b] = ((int)tile - 1 - b >= 0) ? ld_relaxed(st - (size_t)(b + 1) * 256) : LB_INC;
 
         uint32_t inc = count;                                       // tile counts over digits
         uint32_t hcount = hist[tid], hinc = hcount;                 // whole-array counts over digits
@@ -112,42 +119,58 @@ onesweep_kernel(uint32_t n, const uint2 *__restrict__ in, uint2 *__restrict__ ou
         if (lane == 31) { S.scan_tmp[warp] = inc; S.scan_tmp[8 + warp] = hinc; }
         exc_in_warp = inc - count;
         hexc_in_warp = hinc - hcount;
-
-        if (tile > 0) {                                             // same digit in earlier tiles
-            int t = (int)tile - 1;
-            while (true) {
-                uint32_t v = ld_relaxed(tile_state + (size_t)t * 256 + tid);
-                uint32_t f = v >> 30;
-                if (f == 0) continue;
-                lookback += v & LB_VAL;
-                if (f == 2) break;
-                --t;
-            }
-            st_relaxed(st, LB_INC | (lookback + count));
-        }
     }
     __syncthreads();
     if (tid < 256) {
-        uint32_t add = 0, hadd = 0;
+        uint32_t dstart = 0, hadd = 0;
 #pragma unroll
         for (int w = 0; w < 8; ++w) {
-            add += (w < (int)warp) ? S.scan_tmp[w] : 0u;
+            dstart += (w < (int)warp) ? S.scan_tmp[w] : 0u;
             hadd += (w < (int)warp) ? S.scan_tmp[8 + w] : 0u;
         }
-        uint32_t dstart = exc_in_warp + add;
+        dstart += exc_in_warp;
         S.digit_start[tid] = dstart;
-        S.gbase[tid] = hexc_in_warp + hadd + lookback - dstart;
+        S.gbase[tid] = hexc_in_warp + hadd - dstart;    // + look-back, added below
     }
     __syncthreads();
 
-    // ---- reorder the tile through shared memory
+    // ---- reorder the tile through shared memory (needs only tile-local offsets)
 #pragma unroll
     for (int k = 0; k < RS_IPT; ++k) {
         uint32_t li = wbase + k * 32 + lane;
         if (li < tile_n) {
             uint32_t d = (kv[k].x >> shift) & dmask;
-            S.stage[S.digit_start[d] + wh[d] + rank[k]] = kv[k];
+            const uint32_t r = (k & 1) ? (rank2[k >> 1] >> 16) : (rank2[k >> 1] & 0xFFFFu);
+            S.stage[S.digit_start[d] + wh[d] + r] = kv[k];
         }
+    }
+
+    // ---- finish the look-back: same digit in earlier tiles, RS_LB polls per round
+    if (tid < 256) {
+        uint32_t lookback = 0;
+        if (tile > 0) {
+            int t = (int)tile - 1;
+            bool done = false;
+            while (true) {
+                bool open = true;                                   // no unpublished predecessor met yet
+#pragma unroll
+                for (int b = 0; b < RS_LB; ++b) {
+                    const uint32_t f = poll[b] >> 30;
+                    open = open && (f != 0) && !done;
+                    if (open) {
+                        lookback += poll[b] & LB_VAL;
+                        --t;
+                        done = (f == 2);
+                    }
+                }
+                if (done) break;
+#pragma unroll
+                for (int b = 0; b < RS_LB; ++b)
+                    poll[b] = (t - b >= 0) ? ld_relaxed(tile_state + (size_t)(t - b) * 256 + tid) : LB_INC;
+            }
+            st_relaxed(st, LB_INC | (lookback + count));
+        }
+        S.gbase[tid] += lookback;
     }
     __syncthreads();
     // ---- runs of equal digits go to consecutive global addresses
