@@ -220,18 +220,15 @@ def main():
         return
 
     import torch
-    import torch.distributed as dist
     from paper_1210_1017_b200 import binding as B      # fails loudly without the CUDA library
+    from paper_1210_1017_b200 import replicas as R
     from paper_1210_1017_b200 import workloads as W
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    rep = R.init("nccl")
+    rank, world, local = rep.rank, rep.world, rep.local_rank
     torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     pk = peaks()
 
     nb = CONFIG_NB[args.config]
@@ -245,10 +242,7 @@ def main():
     passes = (v.cell_bits + 7) // 8
 
     def barrier():
-        torch.cuda.synchronize()
-        if world > 1:
-            dist.barrier()
-            torch.cuda.synchronize()
+        R.barrier(rep)
 
     # ---- warm-up
     for _ in range(args.warmup):
@@ -276,11 +270,8 @@ def main():
     sph.sph_profile_enable(False)
     launches = sph.sph_launch_count() - launches0
     assert sph.sph_status() == 0, "non-finite state during the timed run"
-    if world > 1:
-        t = torch.tensor([ms_total], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
-    value = world * n * args.steps / (ms_total * 1e-3) / 1e6
+    rate, ms_total = R.aggregate_rate(rep, float(n) * args.steps, ms_total)   # all replicas / slowest rank
+    value = rate / 1e6
 
     # ---- end-to-end through the C ABI with HOST buffers: upload, step, download, every step
     pin = dict(pos=torch.from_numpy(w.pos).pin_memory(), vel=torch.from_numpy(w.vel).pin_memory(),
@@ -302,17 +293,13 @@ def main():
         e2e_step()
     torch.cuda.synchronize()
     e2e_s = max(time.perf_counter() - t0, 1e-9)
-    if world > 1:
-        t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = R.max_over_ranks(rep, e2e_s)
     e2e = dict(value=world * n * args.e2e_steps / e2e_s / 1e6, unit="Mparticle-steps/s",
                h2d_bytes_per_step=int(n * (12 + 12 + 4 + 1)), d2h_bytes_per_step=int(n * (12 + 12 + 4)),
                steps=args.e2e_steps, api="sph_set_state(host) + sph_step + sph_download(host), pinned buffers")
 
     if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
+        R.finalize(rep)
         return
 
     # ---- roofline of the dominant kernel (interaction): plain FP32 ALUs
@@ -367,8 +354,7 @@ def main():
         sort_gkeys_s=n / (stages["sort"]["ms"] * 1e-3) / 1e9 if "sort" in stages else None,
         stages=stages, hbm_peak_gbs=pk["hbm_gbs"], peak_source=pk["source"])
     print(json.dumps(line))
-    if world > 1:
-        dist.destroy_process_group()
+    R.finalize(rep)
 
 
 if __name__ == "__main__":
