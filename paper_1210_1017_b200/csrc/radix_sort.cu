@@ -6,7 +6,8 @@
 //
 // One kernel per 8-bit digit.  The digit histograms come from the key kernel (keys.cu); each
 // pass is a single sweep: a CTA takes a tile in launch order (dynamic tile id), ranks its keys
-// with a warp-level match (ballots) + per-warp shared-memory counters (stable), publishes its 256 digit
+// with a warp-level match built in shared memory (one atomic OR per key) + per-warp
+// shared-memory counters (stable), publishes its 256 digit
 // counts, resolves the exclusive prefix over earlier tiles by decoupled look-back, reorders the
 // tile through shared memory and writes runs of equal digits to consecutive addresses.
 //
@@ -39,54 +40,66 @@ __device__ __forceinline__ void st_relaxed(uint32_t *p, uint32_t v)
 
 struct __align__(16) RsSmem {
     uint2 stage[RS_TILE];                 // 48 KB
-    uint32_t warp_hist[RS_WARPS][256];    // 16 KB
+    uint2 wm[RS_WARPS][256];              // 32 KB: per warp and digit, .x = match mask of the row being
+                                          // ranked (scratch, 0 between rows), .y = running count
     uint32_t digit_start[256];            // first tile-local slot of each digit
     uint32_t gbase[256];                  // global slot of tile-local slot 0 of each digit
     uint32_t scan_tmp[16];
     uint32_t tile;
 };
 
-__global__ void __launch_bounds__(RS_THREADS, 2)
-onesweep_kernel(uint32_t n, const uint2 *__restrict__ in, uint2 *__restrict__ out,
-                const uint32_t *__restrict__ hist, uint32_t *tile_state, uint32_t *tile_counter, int shift,
-                uint32_t dmask /* keeps the tag bits 28..31 out of the last digit */)
+// Stable warp-level ranking of one row (32 items, one per lane) on an 8-bit digit.  The set of
+// lanes holding the same digit is built in shared memory: every lane ORs its lane bit into the
+// (warp, digit) mask word - OR commutes, so the result does not depend on the order in which the
+// hardware serialises lanes that hit the same word - and reads the word back together with the
+// running count of that digit in earlier rows of the warp.  One ATOMS + one LDS.64 + one STS.64
+// replace the eight ballots (about 50 ALU-pipe instructions) of a register-only match.
+__device__ __forceinline__ uint32_t rank_row(uint32_t wm_warp /* shared address of S.wm[warp] */, uint32_t d,
+                                             uint32_t lane_bit, uint32_t lt_mask)
 {
-    extern __shared__ __align__(16) unsigned char rs_raw[];
-    RsSmem &S = *reinterpret_cast<RsSmem *>(rs_raw);
+    const uint32_t e = wm_warp + 8u * d;
+    uint32_t mx, my;
+    asm volatile("red.shared.or.b32 [%0], %1;" ::"r"(e), "r"(lane_bit) : "memory");
+    __syncwarp();
+    asm volatile("ld.shared.v2.u32 {%0,%1}, [%2];" : "=r"(mx), "=r"(my) : "r"(e) : "memory");
+    __syncwarp();
+    const uint32_t below = mx & lt_mask;
+    if (below == 0)                                                    // lowest lane of the set
+        asm volatile("st.shared.v2.u32 [%0], {%1,%2};" ::"r"(e), "r"(0u), "r"(my + __popc(mx)) : "memory");
+    __syncwarp();
+    return my + __popc(below);
+}
+
+template <bool FULL>
+__device__ __forceinline__ void onesweep_tile(RsSmem &S, uint32_t n, const uint2 *__restrict__ in,
+                                              uint2 *__restrict__ out, const uint32_t *__restrict__ hist,
+                                              uint32_t *tile_state, int shift, uint32_t dmask, uint32_t tile)
+{
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const uint32_t lt_mask = (1u << lane) - 1u;
-
-    if (tid == 0) S.tile = atomicAdd(tile_counter, 1u);
-    for (int k = tid; k < RS_WARPS * 256; k += RS_THREADS) (&S.warp_hist[0][0])[k] = 0;
-    __syncthreads();
-    const uint32_t tile = S.tile;
+    const uint32_t lane_bit = 1u << lane, lt_mask = lane_bit - 1u;
     const uint32_t base = tile * RS_TILE;
-    const uint32_t tile_n = min((uint32_t)RS_TILE, n - base);
+    const uint32_t tile_n = FULL ? (uint32_t)RS_TILE : n - base;
 
-    // ---- load, warp-striped: the warp owns a contiguous chunk; item k of lane l is chunk[k*32+l]
+    // ---- load, warp-striped: the warp owns a contiguous chunk; item k of lane l is chunk[k*32+l].
+    // Slots past the end of the array hold the key 0xFFFFFFFF: its digit is dmask, the largest digit
+    // of the pass, and a stable ranking puts those slots after every real pair of the tile, i.e. at
+    // staged positions >= tile_n, which are never written out.
     uint2 kv[RS_IPT];
-    uint32_t rank2[RS_IPT / 2];                   // warp-local ranks, two 16-bit values per word
     const uint32_t wbase = warp * (32 * RS_IPT);
 #pragma unroll
     for (int k = 0; k < RS_IPT; ++k) {
-        uint32_t li = wbase + k * 32 + lane;
-        kv[k] = li < tile_n ? __ldcs(in + base + li) : make_uint2(0xFFFFFFFFu, 0u);
+        const uint32_t li = wbase + k * 32 + lane;
+        kv[k] = (FULL || li < tile_n) ? __ldcs(in + base + li) : make_uint2(0xFFFFFFFFu, 0u);
     }
-    // ---- rank inside the warp, stable in item order
-    uint32_t *wh = S.warp_hist[warp];
+    // ---- rank inside the warp, stable in item order; two 16-bit ranks per register
+    uint32_t rank2[RS_IPT / 2];
+    const uint32_t wm_addr = (uint32_t)__cvta_generic_to_shared(S.wm[warp]);
+    const uint2 *wm_warp = S.wm[warp];
 #pragma unroll
     for (int k = 0; k < RS_IPT; ++k) {
-        uint32_t li = wbase + k * 32 + lane;
-        bool valid = li < tile_n;
-        uint32_t d = (kv[k].x >> shift) & dmask;
-        uint32_t m = warp_match8(d, valid);
-        uint32_t leader = __ffs(m) - 1;
-        uint32_t old = 0;
-        if (valid && lane == leader) { old = wh[d]; wh[d] = old + __popc(m); }
-        old = __shfl_sync(0xffffffffu, old, leader);
-        const uint32_t r = old + __popc(m & lt_mask);
+        const uint32_t d = (kv[k].x >> shift) & dmask;
+        const uint32_t r = rank_row(wm_addr, d, lane_bit, lt_mask);
         if (k & 1) rank2[k >> 1] |= r << 16; else rank2[k >> 1] = r;
-        __syncwarp();
     }
     __syncthreads();
 
@@ -99,11 +112,13 @@ onesweep_kernel(uint32_t n, const uint2 *__restrict__ in, uint2 *__restrict__ ou
     if (tid < 256) {
 #pragma unroll
         for (int w = 0; w < RS_WARPS; ++w) {
-            uint32_t t = S.warp_hist[w][tid];
-            S.warp_hist[w][tid] = count;
+            const uint32_t t = S.wm[w][tid].y;
+            S.wm[w][tid].y = count;
             count += t;
         }
-        st_relaxed(st, (tile == 0 ? LB_INC : LB_AGG) | count);
+        const uint32_t pads = FULL ? 0u : (tid == dmask ? (uint32_t)RS_TILE - tile_n : 0u);
+        const uint32_t pub = count - pads;                         // real pairs of this digit in the tile
+        st_relaxed(st, (tile == 0 ? LB_INC : LB_AGG) | pub);
 #pragma unroll
         for (int b = 0; b < RS_LB; ++b)
             poll[b] = ((int)tile - 1 - b >= 0) ? ld_relaxed(st - (size_t)(b + 1) * 256) : LB_INC;
@@ -119,6 +134,7 @@ onesweep_kernel(uint32_t n, const uint2 *__restrict__ in, uint2 *__restrict__ ou
         if (lane == 31) { S.scan_tmp[warp] = inc; S.scan_tmp[8 + warp] = hinc; }
         exc_in_warp = inc - count;
         hexc_in_warp = hinc - hcount;
+        count = pub;
     }
     __syncthreads();
     if (tid < 256) {
@@ -137,12 +153,9 @@ onesweep_kernel(uint32_t n, const uint2 *__restrict__ in, uint2 *__restrict__ ou
     // ---- reorder the tile through shared memory (needs only tile-local offsets)
 #pragma unroll
     for (int k = 0; k < RS_IPT; ++k) {
-        uint32_t li = wbase + k * 32 + lane;
-        if (li < tile_n) {
-            uint32_t d = (kv[k].x >> shift) & dmask;
-            const uint32_t r = (k & 1) ? (rank2[k >> 1] >> 16) : (rank2[k >> 1] & 0xFFFFu);
-            S.stage[S.digit_start[d] + wh[d] + r] = kv[k];
-        }
+        const uint32_t d = (kv[k].x >> shift) & dmask;
+        const uint32_t r = (k & 1) ? (rank2[k >> 1] >> 16) : (rank2[k >> 1] & 0xFFFFu);
+        S.stage[S.digit_start[d] + wm_warp[d].y + r] = kv[k];
     }
 
     // ---- finish the look-back: same digit in earlier tiles, RS_LB polls per round
@@ -176,13 +189,32 @@ onesweep_kernel(uint32_t n, const uint2 *__restrict__ in, uint2 *__restrict__ ou
     // ---- runs of equal digits go to consecutive global addresses
 #pragma unroll
     for (int k = 0; k < RS_IPT; ++k) {
-        uint32_t i = tid + k * RS_THREADS;
-        if (i < tile_n) {
-            uint2 e = S.stage[i];
-            uint32_t d = (e.x >> shift) & dmask;
+        const uint32_t i = tid + k * RS_THREADS;
+        if (FULL || i < tile_n) {
+            const uint2 e = S.stage[i];
+            const uint32_t d = (e.x >> shift) & dmask;
             out[S.gbase[d] + i] = e;
         }
     }
+}
+
+__global__ void __launch_bounds__(RS_THREADS, 2)
+onesweep_kernel(uint32_t n, const uint2 *__restrict__ in, uint2 *__restrict__ out,
+                const uint32_t *__restrict__ hist, uint32_t *tile_state, uint32_t *tile_counter, int shift,
+                uint32_t dmask /* keeps the tag bits 28..31 out of the last digit */)
+{
+    extern __shared__ __align__(16) unsigned char rs_raw[];
+    RsSmem &S = *reinterpret_cast<RsSmem *>(rs_raw);
+    const uint32_t tid = threadIdx.x;
+    if (tid == 0) S.tile = atomicAdd(tile_counter, 1u);
+    {
+        uint4 *z = reinterpret_cast<uint4 *>(&S.wm[0][0]);
+        for (int k = tid; k < RS_WARPS * 256 / 2; k += RS_THREADS) z[k] = make_uint4(0u, 0u, 0u, 0u);
+    }
+    __syncthreads();
+    const uint32_t tile = S.tile;
+    if ((uint64_t)(tile + 1) * RS_TILE <= n) onesweep_tile<true>(S, n, in, out, hist, tile_state, shift, dmask, tile);
+    else onesweep_tile<false>(S, n, in, out, hist, tile_state, shift, dmask, tile);
 }
 
 cudaError_t launch_sort(sph_ctx *c)
