@@ -5,138 +5,122 @@
 //
 // gather_kernel: one thread per sorted slot j; reads the sorted (keyword, source) pair, gathers
 // pos4 / velrho4 / velrhoM1 / idt from the previous order (the source index is close to j in a
-// running simulation, so the gather is L2-friendly), writes them contiguously, writes the
-// sorted keyword array and marks cell_begin[c] = j where a run of cell c starts.
-// cell_fill_kernel: one chained suffix-min scan (decoupled look-back) gives every empty cell
-// the begin of the next non-empty one, i.e. lower_bound semantics for all cells.
-// HBM-bound: 8 + 52 B read, 56 B written per particle; 8 B per cell.
+// running simulation, so the gather is L2-friendly), writes them contiguously and writes the
+// sorted keyword array.  The cell table is written by the same threads: where a run of cell c
+// starts at slot j, every cell in (previous cell, c] gets cell_begin = j (lower_bound semantics
+// for empty cells, reading A11).  Gaps of up to GAP_INLINE cells are filled by the
+// thread itself; longer ones (the empty part of the tank) go on a work list that
+// gap_fill_kernel fills one CTA per chunk.  No memset and no scan over the table: every entry is
+// written exactly once.  The kernel also counts the migrants of its 256 slots (a6).
+// HBM-bound: 8 + 52 B read, 56 B written per particle; 4 B written per cell.
 #include "sph_internal.cuh"
 
 namespace sph {
 
-__global__ void __launch_bounds__(256)
-gather_kernel(uint32_t n, const uint2 *__restrict__ kv,
+constexpr uint32_t GAP_INLINE = 32;        // cells a thread fills itself
+constexpr uint32_t GAP_CHUNK = 1u << 16;   // cells per work-list entry
+
+__device__ __forceinline__ void fill_cells(uint32_t lo, uint32_t hi /* inclusive */, uint32_t value,
+                                           uint32_t *__restrict__ cell_begin, uint4 *__restrict__ gap_list,
+                                           uint32_t *__restrict__ gap_count)
+{
+    if (hi - lo < GAP_INLINE) {
+        for (uint32_t cc = lo; cc <= hi; ++cc) cell_begin[cc] = value;
+    } else {
+        for (uint32_t a = lo; a <= hi; a += GAP_CHUNK) {
+            const uint32_t b = min(hi, a + (GAP_CHUNK - 1u));
+            gap_list[atomicAdd(gap_count, 1u)] = make_uint4(a, b, value, 0u);
+            if (b == hi) break;              // a + GAP_CHUNK could wrap for hi near 2^32
+        }
+    }
+}
+
+__global__ void __launch_bounds__(GATHER_THREADS)
+gather_kernel(uint32_t n, uint32_t ncells, const uint2 *__restrict__ kv,
               const float4 *__restrict__ pos_in, const float4 *__restrict__ vr_in,
               const float4 *__restrict__ vm_in, const uint32_t *__restrict__ idt_in,
               float4 *__restrict__ pos_out, float4 *__restrict__ vr_out, float4 *__restrict__ vm_out,
               uint32_t *__restrict__ idt_out, uint32_t *__restrict__ keyword,
-              uint32_t *__restrict__ cell_begin)
+              uint32_t *__restrict__ cell_begin, uint4 *__restrict__ gap_list, uint32_t *__restrict__ gap_count,
+              uint32_t *__restrict__ mig_tile, uint32_t *__restrict__ mig_grp)
 {
-    uint32_t j = blockIdx.x * blockDim.x + threadIdx.x;
-    if (j >= n) return;
-    uint2 e = __ldcs(kv + j);
-    uint32_t src = e.y & 0x0FFFFFFFu;
-    uint32_t cell = e.x & CELL_MASK;
-    uint32_t prev_cell = j ? (kv[j - 1].x & CELL_MASK) : 0xFFFFFFFFu;
-    float4 p = pos_in[src];
-    float4 v = vr_in[src];
-    float4 m = vm_in[src];
-    uint32_t w = idt_in[src];
-    __stcs(pos_out + j, p);       // streamed: re-read by later kernels but not by this one
-    __stcs(vr_out + j, v);
-    __stcs(vm_out + j, m);
-    idt_out[j] = w;
-    keyword[j] = e.x;
-    if (cell != prev_cell) cell_begin[cell] = j;
+    const uint32_t j = blockIdx.x * blockDim.x + threadIdx.x;
+    bool migrant = false;
+    if (j < n) {
+        const uint2 e = __ldcs(kv + j);
+        const uint32_t src = e.y & 0x0FFFFFFFu;
+        const uint32_t cell = e.x & CELL_MASK;
+        const float4 p = pos_in[src];
+        const float4 v = vr_in[src];
+        const float4 m = vm_in[src];
+        const uint32_t w = idt_in[src];
+        __stcs(pos_out + j, p);       // streamed: re-read by later kernels but not by this one
+        __stcs(vr_out + j, v);
+        __stcs(vm_out + j, m);
+        idt_out[j] = w;
+        keyword[j] = e.x;
+        migrant = (e.x >> 30) != 0;
+        if (j == 0) {
+            fill_cells(0u, cell, 0u, cell_begin, gap_list, gap_count);
+        } else {
+            const uint32_t prev_cell = kv[j - 1].x & CELL_MASK;
+            if (cell != prev_cell) fill_cells(prev_cell + 1u, cell, j, cell_begin, gap_list, gap_count);
+        }
+        if (j == n - 1) fill_cells(cell + 1u, ncells, n, cell_begin, gap_list, gap_count);   // incl. the sentinel
+    }
+    const int cnt = __syncthreads_count(migrant);
+    if (threadIdx.x == 0) {
+        mig_tile[blockIdx.x] = (uint32_t)cnt;
+        if (cnt) atomicAdd(&mig_grp[blockIdx.x / MG_SUB], (uint32_t)cnt);     // group of MG_SUB tiles
+    }
 }
+
+// One CTA per work-list entry (grid-stride): cell_begin[lo..hi] = value.
+__global__ void __launch_bounds__(256)
+gap_fill_kernel(const uint4 *__restrict__ gap_list, const uint32_t *__restrict__ gap_count,
+                uint32_t *__restrict__ cell_begin)
+{
+    const uint32_t count = *gap_count;
+    for (uint32_t e = blockIdx.x; e < count; e += gridDim.x) {
+        const uint4 g = gap_list[e];
+        for (uint32_t cc = g.x + threadIdx.x; cc <= g.y; cc += blockDim.x) cell_begin[cc] = g.z;
+    }
+}
+
+uint32_t mig_groups(uint64_t n) { return (gather_tiles(n) + MG_SUB - 1) / MG_SUB; }
+uint32_t gather_tiles(uint64_t n) { return (uint32_t)((n + GATHER_THREADS - 1) / GATHER_THREADS); }
+size_t gap_list_entries(uint64_t ncells) { return (size_t)(ncells / GAP_INLINE + ncells / GAP_CHUNK + 8); }
 
 cudaError_t launch_gather_cells(sph_ctx *c)
 {
     uint32_t n = (uint32_t)c->n;
-    // unset cells = 0xFFFFFFFF; sentinel cell_begin[ncells] = n
-    cudaError_t e = cudaMemsetAsync(c->cell_begin, 0xFF, sizeof(uint32_t) * ((size_t)c->grid.ncells + 1), c->stream);
+    uint32_t *gap_count = c->counters + 8;
+    cudaError_t e = cudaMemsetAsync(gap_count, 0, sizeof(uint32_t), c->stream);
     if (e != cudaSuccess) return e;
     if (n) {
+        e = cudaMemsetAsync(c->mig_grp, 0, sizeof(uint32_t) * ((size_t)mig_groups(n) + 1), c->stream);
+        if (e != cudaSuccess) return e;
         int o = 1 - c->cur;
-        gather_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(
-            n, c->kv[c->kv_sorted], c->pos4[c->cur], c->velrho4[c->cur], c->velrhoM1[c->cur], c->idt[c->cur],
-            c->pos4[o], c->velrho4[o], c->velrhoM1[o], c->idt[o], c->keyword, c->cell_begin);
+        gather_kernel<<<gather_tiles(n), GATHER_THREADS, 0, c->stream>>>(
+            n, c->grid.ncells, c->kv[c->kv_sorted], c->pos4[c->cur], c->velrho4[c->cur], c->velrhoM1[c->cur],
+            c->idt[c->cur], c->pos4[o], c->velrho4[o], c->velrhoM1[o], c->idt[o], c->keyword, c->cell_begin,
+            c->gap_list, gap_count, c->mig_tile, c->mig_grp);
         c->n_launches++;
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;
         c->cur = o;
+    } else {
+        // no particles: every entry, sentinel included, is 0
+        e = cudaMemsetAsync(c->cell_begin, 0, sizeof(uint32_t) * ((size_t)c->grid.ncells + 1), c->stream);
     }
-    return cudaSuccess;
+    return e;
 }
 
-// ---- suffix-min scan over cell_begin[0..ncells] -----------------------------------------------
-constexpr int CF_THREADS = 256;
-constexpr int CF_IPT = 16;
-constexpr int CF_TILE = CF_THREADS * CF_IPT;
-uint32_t scan_tiles(uint64_t n) { return (uint32_t)((n + CF_TILE - 1) / CF_TILE); }
-
-// Tiles are numbered from the END of the array (tile 0 holds the last elements), so that the
-// suffix scan is a forward chained scan over tiles.  state word: flag<<32 | value.
-__global__ void __launch_bounds__(CF_THREADS)
-cell_fill_kernel(uint32_t m /* ncells+1 */, uint32_t n, uint32_t *__restrict__ cell_begin,
-                 unsigned long long *state, uint32_t *ticket)
-{
-    __shared__ uint32_t s_tile, s_warp_min[CF_THREADS / 32], s_carry;
-    const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    if (tid == 0) s_tile = atomicAdd(ticket, 1u);
-    __syncthreads();
-    const uint32_t tile = s_tile;
-    // element index of reversed position q: idx = m-1-q ; thread handles CF_IPT consecutive q
-    const uint32_t q0 = tile * CF_TILE + tid * CF_IPT;
-    uint32_t v[CF_IPT];
-#pragma unroll
-    for (int k = 0; k < CF_IPT; ++k) {
-        uint32_t q = q0 + k;
-        v[k] = 0xFFFFFFFFu;
-        if (q < m) v[k] = (q == 0) ? n : cell_begin[m - 1 - q];
-    }
-    // inclusive running min in reversed order inside the thread
-#pragma unroll
-    for (int k = 1; k < CF_IPT; ++k) v[k] = min(v[k], v[k - 1]);
-    uint32_t tmin = v[CF_IPT - 1];
-    // exclusive scan (min) over threads
-    uint32_t inc = tmin;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
-        if (lane >= (uint32_t)o) inc = min(inc, t);
-    }
-    uint32_t exc = __shfl_up_sync(0xffffffffu, inc, 1);
-    if (lane == 0) exc = 0xFFFFFFFFu;
-    if (lane == 31) s_warp_min[warp] = inc;
-    __syncthreads();
-    uint32_t wpre = 0xFFFFFFFFu, block_min = 0xFFFFFFFFu;
-#pragma unroll
-    for (int w = 0; w < CF_THREADS / 32; ++w) {
-        uint32_t t = s_warp_min[w];
-        if (w < (int)warp) wpre = min(wpre, t);
-        block_min = min(block_min, t);
-    }
-    exc = min(exc, wpre);
-    // chained look-back over earlier tiles (= later cells), warp 0, 32 tiles per round trip
-    if (warp == 0) {
-        if (lane == 0) st_relaxed_u64(state + tile, ((tile == 0 ? 2ull : 1ull) << 32) | block_min);
-        uint32_t carry = 0xFFFFFFFFu;
-        if (tile > 0) {
-            carry = warp_lookback(state, tile, 0xFFFFFFFFu, [](uint32_t a, uint32_t b) { return min(a, b); });
-            if (lane == 0) st_relaxed_u64(state + tile, (2ull << 32) | min(carry, block_min));
-        }
-        if (lane == 0) s_carry = carry;
-    }
-    __syncthreads();
-    exc = min(exc, s_carry);
-#pragma unroll
-    for (int k = 0; k < CF_IPT; ++k) {
-        uint32_t q = q0 + k;
-        if (q < m) cell_begin[m - 1 - q] = min(v[k], exc);
-    }
-}
-
+// long gaps of the cell table (work list written by gather_kernel)
 cudaError_t launch_cell_fill(sph_ctx *c)
 {
-    uint32_t m = c->grid.ncells + 1;
-    uint32_t tiles = scan_tiles(m);
-    cudaError_t e = cudaMemsetAsync(c->scan_state, 0, sizeof(unsigned long long) * tiles, c->stream);
-    if (e != cudaSuccess) return e;
-    e = cudaMemsetAsync(c->counters + 8, 0, sizeof(uint32_t), c->stream);
-    if (e != cudaSuccess) return e;
-    cell_fill_kernel<<<tiles, CF_THREADS, 0, c->stream>>>(m, (uint32_t)c->n, c->cell_begin, c->scan_state,
-                                                        c->counters + 8);
+    if (c->n == 0) return cudaSuccess;
+    gap_fill_kernel<<<NUM_SMS * 4, 256, 0, c->stream>>>(c->gap_list, c->counters + 8, c->cell_begin);
     c->n_launches++;
     return cudaGetLastError();
 }

@@ -46,88 +46,122 @@ cudaError_t launch_halo_gather(sph_ctx *c)
     return cudaGetLastError();
 }
 
-// ---- migrants: ordered stream compaction (chained scan with decoupled look-back) -----------------
-constexpr int MG_THREADS = 256;
-constexpr int MG_IPT = 16;
-constexpr int MG_TILE = MG_THREADS * MG_IPT;
+// ---- migrants: ordered stream compaction in three steps without any inter-CTA wait ----------------
+//  1. gather_kernel (gather_cells.cu) already counted the migrants of every 256-slot tile while it had
+//     the sorted keywords in registers (mig_tile[t]) and of every group of MG_SUB tiles (mig_grp[g]);
+//  2. mig_scan_kernel: exclusive scan of the group counts in place (one CTA; the array has n/4096
+//     entries), total -> mig_total;
+//  3. mig_compact_kernel: a CTA owns MG_SUB consecutive tiles, skips them when they hold no migrant
+//     (in a running simulation migrants exist only next to the slab planes), otherwise re-reads the
+//     keywords, ranks the flagged slots with ballots and writes the records in sorted order.
+constexpr int MG_SCAN_THREADS = 1024;
 
-__global__ void __launch_bounds__(MG_THREADS)
-migrants_kernel(uint32_t n, const uint32_t *__restrict__ keyword, const uint2 *__restrict__ kv,
-                const uint32_t *__restrict__ idt, SlabC sl, int nyz, unsigned long long *state,
-                uint32_t *ticket, uint4 *__restrict__ records, uint32_t *__restrict__ mig_total,
-                uint32_t *__restrict__ mig_count)
+__global__ void __launch_bounds__(MG_SCAN_THREADS)
+mig_scan_kernel(uint32_t tiles, uint32_t *__restrict__ mig_tile /* tiles + 1 */, uint32_t *__restrict__ mig_total)
 {
-    __shared__ uint32_t s_tile, s_warp[MG_THREADS / 32], s_carry;
+    __shared__ uint32_t s_warp[MG_SCAN_THREADS / 32];
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    if (tid == 0) s_tile = atomicAdd(ticket, 1u);
+    constexpr uint32_t NW = MG_SCAN_THREADS / 32;
+    // a warp owns a contiguous span; lanes read consecutive entries
+    const uint32_t span = ((tiles + NW - 1) / NW + 31u) & ~31u;
+    const uint32_t lo = warp * span, hi = min(tiles, lo + span);
+    uint32_t sum = 0;
+    for (uint32_t k = lo + lane; k < hi; k += 32) sum += mig_tile[k];
+#pragma unroll
+    for (int o = 16; o; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+    if (lane == 0) s_warp[warp] = sum;
     __syncthreads();
-    const uint32_t tile = s_tile;
-    // blocked arrangement keeps sorted order: thread owns MG_IPT consecutive slots
-    const uint32_t j0 = tile * MG_TILE + tid * MG_IPT;
-    uint32_t flags = 0, cnt = 0;
+    if (warp == 0) {
+        uint32_t v = s_warp[lane], inc = v;
 #pragma unroll
-    for (int k = 0; k < MG_IPT; ++k) {
-        uint32_t j = j0 + k;
-        if (j < n && (keyword[j] >> 30) != 0) { flags |= 1u << k; ++cnt; }
-    }
-    uint32_t inc = cnt;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
-        if (lane >= (uint32_t)o) inc += t;
-    }
-    if (lane == 31) s_warp[warp] = inc;
-    __syncthreads();
-    uint32_t wpre = 0, total = 0;
-#pragma unroll
-    for (int w = 0; w < MG_THREADS / 32; ++w) {
-        uint32_t t = s_warp[w];
-        if (w < (int)warp) wpre += t;
-        total += t;
-    }
-    if (warp == 0) {                     // look-back by warp 0, 32 tiles per round trip
-        if (lane == 0) st_relaxed_u64(state + tile, ((tile == 0 ? 2ull : 1ull) << 32) | total);
-        uint32_t carry = 0;
-        if (tile > 0) {
-            carry = warp_lookback(state, tile, 0u, [](uint32_t a, uint32_t b) { return a + b; });
-            if (lane == 0) st_relaxed_u64(state + tile, (2ull << 32) | (carry + total));
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= (uint32_t)o) inc += t;
         }
-        if (lane == 0) {
-            s_carry = carry;
-            if (tile == gridDim.x - 1) *mig_total = carry + total;   // tiles are ticketed in order
-        }
+        s_warp[lane] = inc - v;
+        if (lane == 31) { *mig_total = inc; mig_tile[tiles] = inc; }
     }
     __syncthreads();
-    uint32_t out = s_carry + wpre + inc - cnt;
-    if (flags) {
+    uint32_t carry = s_warp[warp];
+    for (uint32_t k0 = lo; k0 < hi; k0 += 32) {
+        const uint32_t k = k0 + lane;
+        const uint32_t v = k < hi ? mig_tile[k] : 0u;
+        uint32_t inc = v;
 #pragma unroll
-        for (int k = 0; k < MG_IPT; ++k) {
-            if (flags & (1u << k)) {
-                uint32_t j = j0 + k;
-                uint32_t w = keyword[j];
-                int cx = (int)((w & CELL_MASK) / (uint32_t)nyz);
-                int slab = 0;
-                for (int q = 1; q < sl.n_slabs; ++q) slab += (cx >= sl.planes[q]) ? 1 : 0;
-                uint32_t prev = kv[j].y >> 28;
-                records[out++] = make_uint4(idt[j] & ID_MASK, j, prev, (uint32_t)slab);
-                atomicAdd(&mig_count[2 * prev + ((w >> 30) == 2 ? 1 : 0)], 1u);
-            }
+        for (int o = 1; o < 32; o <<= 1) {
+            uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= (uint32_t)o) inc += t;
+        }
+        if (k < hi) mig_tile[k] = carry + inc - v;
+        carry += __shfl_sync(0xffffffffu, inc, 31);
+    }
+}
+
+__global__ void __launch_bounds__(GATHER_THREADS)
+mig_compact_kernel(uint32_t n, uint32_t tiles, const uint32_t *__restrict__ mig_off,
+                   const uint32_t *__restrict__ mig_tile, const uint32_t *__restrict__ keyword, const uint2 *__restrict__ kv,
+                   const uint32_t *__restrict__ idt, SlabC sl, int nyz, uint4 *__restrict__ records,
+                   uint32_t *__restrict__ mig_count)
+{
+    __shared__ uint32_t s_off[MG_SUB + 1];
+    __shared__ uint32_t s_warp[GATHER_THREADS / 32];
+    __shared__ uint32_t s_cnt[2 * SPH_MAX_SLABS];
+    const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t t0 = blockIdx.x * MG_SUB;
+    const uint32_t g0 = mig_off[blockIdx.x];
+    if (g0 == mig_off[blockIdx.x + 1]) return;             // no migrant in these tiles (CTA-uniform)
+    if (tid == 0) {
+        uint32_t acc = g0;
+        for (int q = 0; q < MG_SUB; ++q) {
+            s_off[q] = acc;
+            acc += (t0 + q < tiles) ? mig_tile[t0 + q] : 0u;
+        }
+        s_off[MG_SUB] = acc;
+    }
+    if (tid < 2 * SPH_MAX_SLABS) s_cnt[tid] = 0;
+    __syncthreads();
+    for (int q = 0; q < MG_SUB; ++q) {
+        const uint32_t o0 = s_off[q];
+        if (o0 == s_off[q + 1]) continue;                  // CTA-uniform
+        const uint32_t j = (t0 + q) * GATHER_THREADS + tid;
+        const uint32_t w = j < n ? __ldg(keyword + j) : 0u;
+        const bool flag = (w >> 30) != 0;
+        const uint32_t bal = __ballot_sync(0xffffffffu, flag);
+        __syncthreads();                                   // s_warp of the previous round consumed
+        if (lane == 0) s_warp[warp] = __popc(bal);
+        __syncthreads();
+        if (flag) {
+            uint32_t out = o0 + __popc(bal & ((1u << lane) - 1u));
+            for (uint32_t k = 0; k < warp; ++k) out += s_warp[k];
+            const int cx = (int)((w & CELL_MASK) / (uint32_t)nyz);
+            int slab = 0;
+            for (int k = 1; k < sl.n_slabs; ++k) slab += (cx >= sl.planes[k]) ? 1 : 0;
+            const uint32_t prev = kv[j].y >> 28;
+            records[out] = make_uint4(__ldg(idt + j) & ID_MASK, j, prev, (uint32_t)slab);
+            atomicAdd(&s_cnt[2 * prev + ((w >> 30) == 2 ? 1 : 0)], 1u);
         }
     }
+    __syncthreads();
+    if (tid < 2 * SPH_MAX_SLABS && s_cnt[tid]) atomicAdd(&mig_count[tid], s_cnt[tid]);
 }
 
 cudaError_t launch_migrants(sph_ctx *c)
 {
     uint32_t n = (uint32_t)c->n;
     if (n == 0) return cudaSuccess;
-    uint32_t tiles = (n + MG_TILE - 1) / MG_TILE;
-    cudaError_t e = cudaMemsetAsync(c->scan_state, 0, sizeof(unsigned long long) * tiles, c->stream);
+    const uint32_t tiles = gather_tiles(n), groups = mig_groups(n);
+    // a fresh copy of the group counts each time: the scan runs in place and halos may be
+    // rebuilt (new planes) without a new sort
+    cudaError_t e = cudaMemcpyAsync(c->mig_off, c->mig_grp, sizeof(uint32_t) * groups, cudaMemcpyDeviceToDevice,
+                                    c->stream);
     if (e != cudaSuccess) return e;
-    e = cudaMemsetAsync(c->counters + 9, 0, sizeof(uint32_t), c->stream);
+    mig_scan_kernel<<<1, MG_SCAN_THREADS, 0, c->stream>>>(groups, c->mig_off, c->mig_total);
+    c->n_launches++;
+    e = cudaGetLastError();
     if (e != cudaSuccess) return e;
-    migrants_kernel<<<tiles, MG_THREADS, 0, c->stream>>>(
-        n, c->keyword, c->kv[c->kv_sorted], c->idt[c->cur], c->tagged_slabs, c->grid.nyz, c->scan_state,
-        c->counters + 9, c->migrants, c->mig_total, c->mig_count);
+    mig_compact_kernel<<<groups, GATHER_THREADS, 0, c->stream>>>(
+        n, tiles, c->mig_off, c->mig_tile, c->keyword, c->kv[c->kv_sorted], c->idt[c->cur], c->tagged_slabs, c->grid.nyz,
+        c->migrants, c->mig_count);
     c->n_launches++;
     return cudaGetLastError();
 }

@@ -131,6 +131,13 @@ interact_simple_kernel(uint32_t n, const float4 *__restrict__ pos4, const float4
 }
 
 // ---- staged production kernel --------------------------------------------------------------------
+#ifndef SPH_IA_PAD
+#define SPH_IA_PAD 0          // extra dynamic shared memory per CTA (occupancy experiments)
+#endif
+#ifndef SPH_IA_DRAIN
+#define SPH_IA_DRAIN 2
+#endif
+constexpr int IA_DRAIN = SPH_IA_DRAIN;   // pairs a lane evaluates per drain round
 constexpr int IA_THREADS = 256;
 constexpr int IA_QCAP = 17;          // stack entries per thread; one entry = hit mask of IA_SUB candidates
 constexpr int IA_SUB = 20;           // candidates tested per stack entry (entry = index << 20 | 20-bit mask)
@@ -294,14 +301,14 @@ interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict
             pair_term<KERNEL, GAMMA7>(dx, dy, dz, r2, vi.x, vi.y, vi.z, vi.w, pi.w, ci, vj, Pj, mj, ph,
                                       ax, ay, az, dr);
         };
-        // one drain round: up to two pending pairs per lane, as two interleaved dependency chains
+        // one drain round: up to IA_DRAIN pending pairs per lane, as interleaved dependency chains
         auto drain_round = [&]() {
-            uint32_t s0, s1;
-            bool ok0, ok1;
-            pop(s0, ok0);
-            pop(s1, ok1);
-            interact(s0, ok0);
-            interact(s1, ok1);
+            uint32_t s[IA_DRAIN];
+            bool ok[IA_DRAIN];
+#pragma unroll
+            for (int q = 0; q < IA_DRAIN; ++q) pop(s[q], ok[q]);
+#pragma unroll
+            for (int q = 0; q < IA_DRAIN; ++q) interact(s[q], ok[q]);
         };
 
         for (uint32_t bstart = 0; bstart < total; bstart += IA_CAP) {
@@ -399,14 +406,14 @@ static cudaError_t launch_staged(sph_ctx *c)
     auto kern = interact_staged_kernel<KERNEL, UNIFORM, GAMMA7>;
     static bool attr_set = false;
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(IaSmem));
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(IaSmem) + SPH_IA_PAD);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
     int zb = c->zblock;
     int nzb = (c->grid.nc[2] + zb - 1) / zb;
     uint64_t blocks = (uint64_t)c->grid.nc[0] * c->grid.nc[1] * nzb;
-    kern<<<(uint32_t)blocks, IA_THREADS, sizeof(IaSmem), c->stream>>>(
+    kern<<<(uint32_t)blocks, IA_THREADS, sizeof(IaSmem) + SPH_IA_PAD, c->stream>>>(
         c->pos4[c->cur], c->velrho4[c->cur], c->idt[c->cur], c->keyword, c->cell_begin, c->acc4, c->grid,
         c->phys, zb, nzb);
     c->n_launches++;

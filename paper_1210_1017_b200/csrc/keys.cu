@@ -128,17 +128,24 @@ keys_kernel(uint32_t n, const float4 *__restrict__ pos4, const uint32_t *__restr
                 const uint32_t tag = lab | (mig << 2);
                 kv_by_id[id] = make_uint2((tag << TAG_SHIFT) | cell, ((uint32_t)prev << 28) | i);
             }
-            // warp-aggregated digit histograms (one shared-memory atomic per distinct digit)
+            // digit histograms in shared memory.  One digit in the whole warp (the usual case for the
+            // upper digits of a running simulation): one atomic.  A few runs of equal digits: hardware
+            // MATCH.ANY (its cost grows with the number of distinct values) and one atomic per run.
+            // Otherwise (random keys): one plain shared-memory atomic per key - with ~28 distinct
+            // digits among 32 lanes they hardly collide, measured 2.4 cycles per warp instruction.
+            const uint32_t vmask = __ballot_sync(0xffffffffu, valid);
 #pragma unroll
             for (int q = 0; q < PASSES; ++q) {
-                const uint32_t d = (cell >> (8 * q)) & 255u;
-                const uint32_t d0 = __shfl_sync(0xffffffffu, d, 0);
-                const uint32_t vmask = __ballot_sync(0xffffffffu, valid);
-                if (__all_sync(0xffffffffu, !valid || d == d0)) {           // one digit in the whole warp
-                    if (lane == 0 && vmask) atomicAdd(&s_hist[q * 256 + d0], __popc(vmask));
-                } else {
-                    const uint32_t m = warp_match8(d, valid);
+                const uint32_t d = valid ? ((cell >> (8 * q)) & 255u) : 256u;
+                const uint32_t prev = __shfl_up_sync(0xffffffffu, d, 1);
+                const uint32_t runs = __ballot_sync(0xffffffffu, d != prev);   // lane 0: compares with itself
+                if (runs == 0) {
+                    if (lane == 0 && vmask) atomicAdd(&s_hist[q * 256 + d], __popc(vmask));
+                } else if (__popc(runs) <= MATCH_MAX_RUNS) {
+                    const uint32_t m = __match_any_sync(0xffffffffu, d);
                     if (valid && (m & lt_mask) == 0) atomicAdd(&s_hist[q * 256 + d], __popc(m));
+                } else if (valid) {
+                    atomicAdd(&s_hist[q * 256 + d], 1u);
                 }
             }
         }

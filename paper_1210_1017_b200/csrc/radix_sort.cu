@@ -16,9 +16,18 @@
 
 namespace sph {
 
-constexpr int RS_THREADS = 512;
-constexpr int RS_IPT = 12;                        // pairs per thread
-constexpr int RS_TILE = RS_THREADS * RS_IPT;      // 6144 pairs = 48 KB staged
+#ifndef SPH_RS_THREADS                            // tuning knobs (nvcc -D...), defaults = measured best
+#define SPH_RS_THREADS 256
+#endif
+#ifndef SPH_RS_IPT
+#define SPH_RS_IPT 32
+#endif
+#ifndef SPH_RS_MINBLOCKS
+#define SPH_RS_MINBLOCKS 2
+#endif
+constexpr int RS_THREADS = SPH_RS_THREADS;        // >= 256 (one thread per digit)
+constexpr int RS_IPT = SPH_RS_IPT;                // pairs per thread (even)
+constexpr int RS_TILE = RS_THREADS * RS_IPT;      // 8192 pairs = 64 KB staged
 constexpr int RS_WARPS = RS_THREADS / 32;
 constexpr int RS_LB = 8;                          // look-back polls in flight per thread
 constexpr uint32_t LB_AGG = 1u << 30;             // look-back word: flag in bits 30..31
@@ -39,8 +48,8 @@ __device__ __forceinline__ void st_relaxed(uint32_t *p, uint32_t v)
 }
 
 struct __align__(16) RsSmem {
-    uint2 stage[RS_TILE];                 // 48 KB
-    uint2 wm[RS_WARPS][256];              // 32 KB: per warp and digit, .x = match mask of the row being
+    uint2 stage[RS_TILE];                 // 64 KB
+    uint2 wm[RS_WARPS][256];              // 16 KB: per warp and digit, .x = match mask of the row being
                                           // ranked (scratch, 0 between rows), .y = running count
     uint32_t digit_start[256];            // first tile-local slot of each digit
     uint32_t gbase[256];                  // global slot of tile-local slot 0 of each digit
@@ -198,7 +207,7 @@ __device__ __forceinline__ void onesweep_tile(RsSmem &S, uint32_t n, const uint2
     }
 }
 
-__global__ void __launch_bounds__(RS_THREADS, 2)
+__global__ void __launch_bounds__(RS_THREADS, SPH_RS_MINBLOCKS)
 onesweep_kernel(uint32_t n, const uint2 *__restrict__ in, uint2 *__restrict__ out,
                 const uint32_t *__restrict__ hist, uint32_t *tile_state, uint32_t *tile_counter, int shift,
                 uint32_t dmask /* keeps the tag bits 28..31 out of the last digit */)

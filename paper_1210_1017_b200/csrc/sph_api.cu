@@ -16,7 +16,7 @@ size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 
 struct Layout {
     size_t pos4[2], velrho4[2], velrhoM1[2], idt[2], acc4, kv[2], keyword, hist, tile_state, counters,
-        cell_begin, scan_state, slab_begin, halo_range, halo_offset, halo_pos4, halo_velrho4, halo_idt,
+        cell_begin, gap_list, mig_tile, mig_grp, mig_off, scratch64, slab_begin, halo_range, halo_offset, halo_pos4, halo_velrho4, halo_idt,
         migrants, mig_total, mig_count, prev_init, flags, total;
 };
 
@@ -62,9 +62,11 @@ bool make_layout(const sph_params *p, uint64_t n, int max_slabs, Layout *L)
     L->tile_state = take((size_t)4 * 256 * tiles * 4);
     L->counters = take(4 * 64);
     L->cell_begin = take(4 * (ncells + 1));
-    uint32_t st = scan_tiles(ncells + 1);
-    uint32_t st2 = scan_tiles(nn);
-    L->scan_state = take(8 * (size_t)(st > st2 ? st : st2));
+    L->gap_list = take(16 * gap_list_entries(ncells));
+    L->mig_tile = take(4 * ((size_t)gather_tiles(nn) + 1));
+    L->mig_grp = take(4 * ((size_t)mig_groups(nn) + 1));
+    L->mig_off = take(4 * ((size_t)mig_groups(nn) + 1));
+    L->scratch64 = take(16);
     L->slab_begin = take(4 * (SPH_MAX_SLABS + 1));
     L->halo_range = take(4 * 4 * SPH_MAX_SLABS);
     L->halo_offset = take(4 * (2 * SPH_MAX_SLABS + 1));
@@ -269,7 +271,11 @@ int sph_init(sph_ctx **out, const sph_params *p, const sph_particles *part, int 
     c->counters = (uint32_t *)(w + L.counters);
     c->rs_tiles = radix_tiles(c->n);
     c->cell_begin = (uint32_t *)(w + L.cell_begin);
-    c->scan_state = (unsigned long long *)(w + L.scan_state);
+    c->gap_list = (uint4 *)(w + L.gap_list);
+    c->mig_tile = (uint32_t *)(w + L.mig_tile);
+    c->mig_grp = (uint32_t *)(w + L.mig_grp);
+    c->mig_off = (uint32_t *)(w + L.mig_off);
+    c->scratch64 = (unsigned long long *)(w + L.scratch64);
     c->slab_begin = (uint32_t *)(w + L.slab_begin);
     c->halo_range = (uint32_t *)(w + L.halo_range);
     c->halo_offset = (uint32_t *)(w + L.halo_offset);
@@ -525,7 +531,7 @@ int sph_pair_stats(sph_ctx *c, uint64_t *out)
     if (!c || !out) return SPH_ERR_ARG;
     if (c->sticky) return c->sticky;
     if (!c->sorted_valid) return SPH_ERR_ORDER;
-    unsigned long long *d = c->scan_state;          // idle between calls
+    unsigned long long *d = c->scratch64;
     CK(c, launch_pair_stats(c, d));
     unsigned long long h[2] = {0, 0};
     CK(c, cudaMemcpyAsync(h, d, 16, cudaMemcpyDeviceToHost, c->stream));

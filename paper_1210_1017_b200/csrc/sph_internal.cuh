@@ -12,6 +12,8 @@ constexpr int TAG_SHIFT = 28;                 // bits 28..29 edge label, 30..31 
 constexpr uint32_t ID_MASK = 0x0FFFFFFFu;     // idt bits 0..27 = id, bit 31 = type
 constexpr uint32_t TYPE_BIT = 0x80000000u;
 constexpr int NUM_SMS = 148;                  // B200
+constexpr int GATHER_THREADS = 256;           // slots per tile of gather_kernel = tile of the migrant counts
+constexpr int MG_SUB = 16;                    // tiles per group = per CTA of the migrant compaction
 
 // sticky device flags
 constexpr uint32_t FLAG_NONFINITE = 1u;
@@ -80,12 +82,15 @@ struct sph_ctx {
     uint32_t *keyword;         // sorted keywords
     uint32_t *hist;            // passes*256 digit histograms
     uint32_t *tile_state;      // passes * rs_tiles * 256 look-back words
-    uint32_t *counters;        // 64 words: dynamic tile counters, scan tickets
+    uint32_t *counters;        // 64 words: dynamic tile counters [0..3], gap work-list counter [8]
     uint32_t rs_tiles;
     // cells / slabs
     uint32_t *cell_begin;      // ncells+1
-    unsigned long long *scan_state;   // look-back words of the cell fill and migrant scans
-    uint32_t scan_tiles_cells, scan_tiles_mig;
+    uint4 *gap_list;           // work list of long runs of empty cells (lo, hi, value, -)
+    uint32_t *mig_tile;        // migrants per 256-slot tile, written by gather_kernel
+    uint32_t *mig_grp;         // migrants per group of MG_SUB tiles, accumulated by gather_kernel
+    uint32_t *mig_off;         // exclusive scan of mig_grp (+ total), rebuilt by every halo build
+    unsigned long long *scratch64;    // 2 words for measurement helpers
     uint32_t *slab_begin;      // max_slabs+1 (current), also "previous owner" ranges of the next sort
     uint32_t *halo_range;      // 2*max_slabs * 2 (begin, count)
     uint32_t *halo_offset;     // 2*max_slabs+1
@@ -130,7 +135,9 @@ cudaError_t launch_download_pack(sph_ctx *c, float *pos3, float *vel3, float *rh
                                  float *drho);
 
 uint32_t radix_tiles(uint64_t n);
-uint32_t scan_tiles(uint64_t n);
+uint32_t gather_tiles(uint64_t n);
+uint32_t mig_groups(uint64_t n);
+size_t gap_list_entries(uint64_t ncells);
 size_t interact_smem_bytes(const sph_ctx *c);
 
 // Tait pressure over rho^2 from rho, fp32, cancellation-free.
