@@ -19,6 +19,7 @@
 //    particle walking the cell table with global loads, as the paper describes it.
 //
 // FP32-ALU bound (no tensor cores: this is not a dense contraction).
+#include <cuda_fp16.h>
 #include "sph_internal.cuh"
 
 namespace sph {
@@ -135,21 +136,32 @@ interact_simple_kernel(uint32_t n, const float4 *__restrict__ pos4, const float4
 #define SPH_IA_PAD 0          // extra dynamic shared memory per CTA (occupancy experiments)
 #endif
 #ifndef SPH_IA_DRAIN
-#define SPH_IA_DRAIN 2
+#define SPH_IA_DRAIN 3
+#endif
+#ifndef SPH_IA_QCAP
+#define SPH_IA_QCAP 11
 #endif
 constexpr int IA_DRAIN = SPH_IA_DRAIN;   // pairs a lane evaluates per drain round
 constexpr int IA_THREADS = 256;
-constexpr int IA_QCAP = 17;          // stack entries per thread; one entry = hit mask of IA_SUB candidates
-constexpr int IA_SUB = 20;           // candidates tested per stack entry (entry = index << 20 | 20-bit mask)
+constexpr int IA_QCAP = SPH_IA_QCAP; // stack entries per thread; one entry = hit mask of one block of IA_BLK candidates
+constexpr int IA_BLK = 16;           // candidates per filter block = per stack entry
 constexpr int IA_ZMAX = 32;          // max cells per z-block
-constexpr int IA_CAP = 2688;         // staged candidates per batch (9 columns x 11 cells x 27 + slack), < 4096
+constexpr int IA_CAP = 2688;         // staged candidates per batch (9 columns x 11 cells x 27 + slack), multiple of 16
+constexpr int IA_NBLK = IA_CAP / IA_BLK;
 constexpr float IA_TINY = 1e-30f;    // r2 floor: a coincident pair (the particle itself) adds exactly 0
+static_assert(IA_CAP % IA_BLK == 0 && IA_NBLK <= 256, "block index must fit 8 bits of a stack entry");
 
+// Shared memory of one CTA.  The filter reads ONLY `hp`: 6 bytes per candidate instead of the 16
+// of an fp32 record - the filter loop is bound by shared-memory bandwidth (ncu: 79 % of the LSU
+// wavefront peak with fp32 records), not by arithmetic.
 struct IaSmem {
-    float4 rel[IA_CAP];                       // position relative to the CTA origin, and its square norm
+    float4 rel[IA_CAP];                       // exact position relative to the CTA origin; w = p/rho^2
     float4 vr[IA_CAP];                        // vx, vy, vz, rho (sign bit = boundary type if masses differ)
-    float pr[IA_CAP];                         // p/rho^2
-    uint32_t stack[IA_QCAP * IA_THREADS];     // [entry][thread]: first candidate index << 20 | hit mask
+    uint4 hp[IA_NBLK * 6];                    // fp16 filter copy: per block of 16 candidates 2 x uint4 of x, of y,
+                                              // of z; half2 word k = (candidate k, candidate k + 8), in units of h
+                                              // about the centre of the CTA's neighbourhood
+    uint32_t stack[IA_QCAP * IA_THREADS];     // [entry][thread]: hit mask (bits 0-7: candidates 0-7 of the block,
+                                              // bits 16-23: candidates 8-15) | block index << 8
     uint32_t cbt[9][IA_ZMAX + 3];             // cell_begin of the 9 columns over [zlo, zhi]
     uint32_t col_vstart[10];                  // virtual start of each column in the concatenation
     uint32_t stage_lo[9], stage_hi[9];        // global index range of the column staged in this batch
@@ -162,16 +174,14 @@ __device__ __forceinline__ void sts_u32(uint32_t addr, uint32_t v)
 {
     asm volatile("st.shared.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
 }
+__device__ __forceinline__ void sts_u16(uint32_t addr, unsigned short v)
+{
+    asm volatile("st.shared.u16 [%0], %1;" ::"r"(addr), "h"(v) : "memory");
+}
 __device__ __forceinline__ uint32_t lds_u32(uint32_t addr)
 {
     uint32_t v;
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
-    return v;
-}
-__device__ __forceinline__ float lds_f32(uint32_t addr)
-{
-    float v;
-    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
     return v;
 }
 __device__ __forceinline__ float4 lds_f4(uint32_t addr)
@@ -179,6 +189,23 @@ __device__ __forceinline__ float4 lds_f4(uint32_t addr)
     float4 v;
     asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
     return v;
+}
+__device__ __forceinline__ uint4 lds_u4(uint32_t addr)
+{
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ __half2 as_h2(uint32_t v) { return *reinterpret_cast<__half2 *>(&v); }
+
+// Hit bits of two candidates (the halves of x, y, z) against one target: squared distance in fp16,
+// in units of h, below the padded threshold.  0xFFFF per half that passes.
+__device__ __forceinline__ uint32_t filt2h(__half2 xi, __half2 yi, __half2 zi, uint32_t x, uint32_t y, uint32_t z,
+                                           __half2 thr)
+{
+    const __half2 dx = __hsub2(xi, as_h2(x)), dy = __hsub2(yi, as_h2(y)), dz = __hsub2(zi, as_h2(z));
+    const __half2 r2 = __hfma2(dz, dz, __hfma2(dy, dy, __hmul2(dx, dx)));
+    return __hlt2_mask(r2, thr);
 }
 
 // Origin of the CTA-relative coordinates along one axis.  x - O is EXACT in fp32 for every staged
@@ -197,10 +224,12 @@ __global__ void __launch_bounds__(IA_THREADS, 2)
 interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict__ velrho4,
                        const uint32_t *__restrict__ idt, const uint32_t *__restrict__ keyword,
                        const uint32_t *__restrict__ cell_begin, float4 *__restrict__ acc4,
-                       GridC g, PhysC ph, int zb, int nzb)
+                       GridC g, PhysC ph, int zb, int nzb, float thr_h /* filter threshold, units of h^2 */,
+                       float zlim /* |z| bound the threshold was derived for, units of h */)
 {
     extern __shared__ __align__(16) unsigned char ia_raw[];
     IaSmem &S = *reinterpret_cast<IaSmem *>(ia_raw);
+    __shared__ uint32_t s_wide;       // some staged particle or target lies outside the fp16 error model
     const int tid = threadIdx.x;
 
     // ---- which z-block
@@ -216,6 +245,7 @@ interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict
 
     const int zlo = max(cz0 - 1, 0), zhi = min(cz1 + 1, g.nc[2]);
     const int nz = zhi - zlo;                                    // <= zb + 2
+    if (tid == 0) s_wide = 0u;
     // ---- cell-begin table of the 9 columns
     for (int k = tid; k < 9 * (nz + 1); k += IA_THREADS) {
         int col = k / (nz + 1), z = k % (nz + 1);
@@ -230,6 +260,12 @@ interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict
     const float ox = rel_origin(fmaf((float)cx, cell, g.min[0]), 4.0f * cell);
     const float oy = rel_origin(fmaf((float)cy, cell, g.min[1]), 4.0f * cell);
     const float oz = rel_origin(fmaf((float)cz0, cell, g.min[2]), (float)(zb + 3) * cell);
+    // centre of the neighbourhood in that frame, and the scale of the fp16 filter copy (units of h):
+    // |x|, |y| <= 3 and |z| <= nz for every particle that lies inside its cell
+    const float inv_h = 2.0f * ph.inv_h_half;
+    const float ccx = fmaf((float)cx + 0.5f, cell, g.min[0]) - ox;
+    const float ccy = fmaf((float)cy + 0.5f, cell, g.min[1]) - oy;
+    const float ccz = fmaf((float)zlo + 0.5f * (float)nz, cell, g.min[2]) - oz;
     __syncthreads();
     if (tid == 0) {
         uint32_t acc = 0;
@@ -244,17 +280,15 @@ interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict
     const uint32_t lane_full = 0xffffffffu;
     const uint32_t rel_base = (uint32_t)__cvta_generic_to_shared(S.rel);
     const uint32_t vr_delta = (uint32_t)__cvta_generic_to_shared(S.vr) - rel_base;
-    const uint32_t pr_base = (uint32_t)__cvta_generic_to_shared(S.pr);
+    const uint32_t hp_base = (uint32_t)__cvta_generic_to_shared(S.hp);
     const uint32_t stk_base = (uint32_t)__cvta_generic_to_shared(S.stack) + 4u * tid;
     constexpr uint32_t STK_STRIDE = 4u * IA_THREADS;
     const uint32_t stk_high = stk_base + STK_STRIDE * (IA_QCAP - 1);   // sp above this = stack full
-    // conservative filter radius: rounding of the expanded form is < 3e-3 h^2
-    const float filt2 = ph.four_h2 + 0.02f * ph.h * ph.h;
 
     for (uint32_t chunk = t_begin; chunk < t_end; chunk += IA_THREADS) {
         const uint32_t i = chunk + tid;
         const bool active = i < t_end;
-        float4 pi = make_float4(ox, oy, oz, 0.f), vi = make_float4(0.f, 0.f, 0.f, 1.f);
+        float4 pi = make_float4(ox + ccx, oy + ccy, oz + ccz, 0.f), vi = make_float4(0.f, 0.f, 0.f, 1.f);
         int kz = 0;
         bool fluid = false;
         if (active) {
@@ -264,8 +298,10 @@ interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict
             kz = (int)((keyword[i] & CELL_MASK) - own_col) - zlo;   // own cz - zlo
         }
         const float xi = pi.x - ox, yi = pi.y - oy, zi = pi.z - oz;  // exact
-        const float fa = -2.0f * xi, fb = -2.0f * yi, fc = -2.0f * zi;
-        const float fT = filt2 - fmaf(zi, zi, fmaf(yi, yi, xi * xi));
+        // fp16 filter copy of the target; a target outside the error model widens the CTA's filter
+        const float xs = (xi - ccx) * inv_h, ys = (yi - ccy) * inv_h, zs = (zi - ccz) * inv_h;
+        if (!(fabsf(xs) < 8.0f && fabsf(ys) < 8.0f && fabsf(zs) < zlim)) s_wide = 1u;
+        const __half2 hxi = __float2half2_rn(xs), hyi = __float2half2_rn(ys), hzi = __float2half2_rn(zs);
         const float ci = sound_speed<GAMMA7>(vi.w, ph);
         const int k_lo = max(kz - 1, 0), k_hi = min(kz + 2, nz);   // own 3-cell window in cbt rows
         float ax = 0.f, ay = 0.f, az = 0.f, dr = 0.f;
@@ -277,20 +313,22 @@ interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict
             if (cur_mask == 0 && sp > stk_base) {
                 sp -= STK_STRIDE;
                 const uint32_t e = lds_u32(sp);
-                cur_mask = e & 0xFFFFFu;
-                cur_s = e >> 20;
+                cur_mask = e & 0x00FF00FFu;
+                cur_s = (e & 0xFF00u) >> 4;                          // block index * 16
             }
             ok = cur_mask != 0;
-            s = cur_s + (uint32_t)(__ffs(cur_mask) - 1);
+            const uint32_t bit = (uint32_t)(__ffs(cur_mask) - 1);    // 0..7 or 16..23 (garbage if !ok)
+            s = cur_s + (bit & 7u) + (bit >> 1 & 8u);
             cur_mask &= cur_mask - 1;
         };
         // pair term of candidate s; ok = false turns it into a no-op without a branch (s = 0 is
-        // always a staged, finite candidate; its mass factor is zeroed)
+        // always a staged, finite candidate; its mass factor is zeroed).  The exact fp32 distance is
+        // formed here: a candidate the fp16 filter let through although it lies outside 2h adds
+        // exactly 0 because F is clamped.
         auto interact = [&](uint32_t s, bool ok) {
             s = ok ? s : 0u;
             const float4 rj = lds_f4(rel_base + 16u * s);
             float4 vj = lds_f4(rel_base + vr_delta + 16u * s);
-            const float Pj = lds_f32(pr_base + 4u * s);
             const float dx = xi - rj.x, dy = yi - rj.y, dz = zi - rj.z;     // == absolute differences
             const float r2 = fmaxf(fmaf(dz, dz, fmaf(dy, dy, dx * dx)), IA_TINY);
             float mj = ok ? 1.0f : 0.0f;
@@ -298,7 +336,7 @@ interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict
                 mj = ok ? (vj.w < 0.f ? ph.mass_bound : ph.mass_fluid) : 0.0f;
                 vj.w = fabsf(vj.w);
             }
-            pair_term<KERNEL, GAMMA7>(dx, dy, dz, r2, vi.x, vi.y, vi.z, vi.w, pi.w, ci, vj, Pj, mj, ph,
+            pair_term<KERNEL, GAMMA7>(dx, dy, dz, r2, vi.x, vi.y, vi.z, vi.w, pi.w, ci, vj, rj.w, mj, ph,
                                       ax, ay, az, dr);
         };
         // one drain round: up to IA_DRAIN pending pairs per lane, as interleaved dependency chains
@@ -336,14 +374,27 @@ interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict
                     float4 v = __ldg(velrho4 + j);
                     if (!UNIFORM && (__ldg(idt + j) & TYPE_BIT)) v.w = -v.w;
                     const float xr = p.x - ox, yr = p.y - oy, zr = p.z - oz;
-                    S.rel[(int32_t)j + off] = make_float4(xr, yr, zr, fmaf(zr, zr, fmaf(yr, yr, xr * xr)));
-                    S.vr[(int32_t)j + off] = v;
-                    S.pr[(int32_t)j + off] = p.w;
+                    const uint32_t si = (uint32_t)((int32_t)j + off);
+                    S.rel[si] = make_float4(xr, yr, zr, p.w);
+                    S.vr[si] = v;
+                    const float xq = (xr - ccx) * inv_h, yq = (yr - ccy) * inv_h, zq = (zr - ccz) * inv_h;
+                    if (!(fabsf(xq) < 8.0f && fabsf(yq) < 8.0f && fabsf(zq) < zlim)) s_wide = 1u;
+                    // block si / 16: x words at +0, y at +32, z at +64; candidate c = si % 16 is half c / 8 of word c % 8
+                    const uint32_t a = hp_base + 96u * (si >> 4) + 4u * (si & 7u) + ((si >> 2) & 2u);
+                    sts_u16(a, __half_as_ushort(__float2half_rn(xq)));
+                    sts_u16(a + 32u, __half_as_ushort(__float2half_rn(yq)));
+                    sts_u16(a + 64u, __half_as_ushort(__float2half_rn(zq)));
                 }
             }
             __syncthreads();
+            // a particle outside the fp16 error model (it left the grid and sits clamped in an edge
+            // cell): let every candidate through, the drain decides exactly
+            const __half2 thr = __float2half2_rn(s_wide ? 65504.0f : thr_h);
 
-            // ---- filter + drain
+            const bool wide = s_wide != 0u;
+
+            // ---- filter + drain.  Blocks of 16 candidates are aligned in shared memory; the first
+            // and the last block of a lane's range are trimmed with masks in the entry's bit layout.
             for (int col = 0; col < 9; ++col) {
                 int lo = 0, hi = 0;
                 if (active) {
@@ -351,38 +402,34 @@ interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict
                     hi = (int)min(S.cbt[col][k_hi], S.stage_hi[col]);
                 }
                 const int off = S.stage_off[col];
-                const int len = max(hi - lo, 0);
-                const int maxlen = __reduce_max_sync(lane_full, len);
-                // lanes without work in this column read from index 0 and record nothing
-                const bool work = len > 0;
-                const int minlen = __reduce_min_sync(lane_full, work ? len : 0x7fffffff);
-                uint32_t s = work ? (uint32_t)(lo + off) : 0u;       // smem index of the next candidate
-                const uint32_t s_hi = s + (uint32_t)len;
-                int sb = 0;
-                // sub-batches of IA_SUB that are complete for every working lane: no range checks.
-                // |r_ij|^2 < R^2  <=>  |r_j|^2 - 2 r_i.r_j < R^2 - |r_i|^2   (3 FFMA + 1 compare)
-                for (; sb + IA_SUB <= minlen && sb < maxlen; sb += IA_SUB, s += IA_SUB) {
-                    uint32_t mask = 0;
-                    const uint32_t a0 = rel_base + 16u * s;
-#pragma unroll
-                    for (int u = 0; u < IA_SUB; ++u) {
-                        const float4 rj = lds_f4(a0 + 16u * u);
-                        if (fmaf(fc, rj.z, fmaf(fb, rj.y, fmaf(fa, rj.x, rj.w))) < fT) mask |= 1u << u;
-                    }
-                    if (work && mask) { sts_u32(sp, (s << 20) | mask); sp += STK_STRIDE; }
-                    while (__any_sync(lane_full, sp > stk_high)) drain_round();
-                }
-                // ragged remainder in groups of 4 with per-lane range checks (reads past s_hi stay
-                // inside the CTA's shared memory: s < IA_CAP and advances by at most IA_CAP)
-                for (; sb < maxlen; sb += 4, s += 4) {
-                    uint32_t mask = 0;
-                    const uint32_t a0 = rel_base + 16u * s;
-#pragma unroll
-                    for (int u = 0; u < 4; ++u) {
-                        const float4 rj = lds_f4(a0 + 16u * u);
-                        if (s + u < s_hi && fmaf(fc, rj.z, fmaf(fb, rj.y, fmaf(fa, rj.x, rj.w))) < fT) mask |= 1u << u;
-                    }
-                    if (mask) { sts_u32(sp, (s << 20) | mask); sp += STK_STRIDE; }
+                const bool work = hi > lo;
+                const uint32_t slo = work ? (uint32_t)(lo + off) : 0u, shi = work ? (uint32_t)(hi + off) : 0u;
+                const uint32_t blk_lo = slo >> 4;
+                const int nblk = work ? (int)(((shi + 15u) >> 4) - blk_lo) : 0;
+                const int maxblk = __reduce_max_sync(lane_full, nblk);
+                uint32_t lin = (0xFFFFu << (slo & 15u)) & 0xFFFFu;                    // candidates >= slo
+                const uint32_t first_mask = (lin & 0xFFu) | ((lin & 0xFF00u) << 8);
+                lin = 0xFFFFu >> ((16u - (shi & 15u)) & 15u);                          // candidates < shi
+                const uint32_t last_mask = (lin & 0xFFu) | ((lin & 0xFF00u) << 8);
+                for (int it = 0; it < maxblk; ++it) {
+                    const uint32_t blk = min(blk_lo + (uint32_t)it, (uint32_t)(IA_NBLK - 1));
+                    const uint32_t a0 = hp_base + 96u * blk;
+                    const uint4 x0 = lds_u4(a0), x1 = lds_u4(a0 + 16u);
+                    const uint4 y0 = lds_u4(a0 + 32u), y1 = lds_u4(a0 + 48u);
+                    const uint4 z0 = lds_u4(a0 + 64u), z1 = lds_u4(a0 + 80u);
+                    uint32_t m;
+                    m = filt2h(hxi, hyi, hzi, x0.x, y0.x, z0.x, thr) & 0x00010001u;
+                    m |= filt2h(hxi, hyi, hzi, x0.y, y0.y, z0.y, thr) & 0x00020002u;
+                    m |= filt2h(hxi, hyi, hzi, x0.z, y0.z, z0.z, thr) & 0x00040004u;
+                    m |= filt2h(hxi, hyi, hzi, x0.w, y0.w, z0.w, thr) & 0x00080008u;
+                    m |= filt2h(hxi, hyi, hzi, x1.x, y1.x, z1.x, thr) & 0x00100010u;
+                    m |= filt2h(hxi, hyi, hzi, x1.y, y1.y, z1.y, thr) & 0x00200020u;
+                    m |= filt2h(hxi, hyi, hzi, x1.z, y1.z, z1.z, thr) & 0x00400040u;
+                    m |= filt2h(hxi, hyi, hzi, x1.w, y1.w, z1.w, thr) & 0x00800080u;
+                    if (wide) m = 0x00FF00FFu;
+                    if (it == 0) m &= first_mask;
+                    if (it == nblk - 1) m &= last_mask;
+                    if (it < nblk && m) { sts_u32(sp, m | (blk << 8)); sp += STK_STRIDE; }
                     while (__any_sync(lane_full, sp > stk_high)) drain_round();
                 }
             }
@@ -400,6 +447,20 @@ interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict
     }
 }
 
+// Filter threshold in units of h^2 for coordinates |x|, |y| < 8 and |z| < zlim (units of h) held in
+// fp16: 4 (= (2h)^2) plus a bound of the error of the fp16 squared distance of any pair with true
+// distance < 2h, rounded up to a multiple of 2^-7.
+static void filter_threshold(int zb, float *thr_h, float *zlim)
+{
+    double zl = 8.0;
+    while (zl < (double)(zb + 2) + 1.0) zl *= 2.0;
+    const double ex = 0.0078125 + 0.001953125;            // two half-ulps below 8 + rounding of the difference
+    const double ez = zl / 2048.0 + 0.001953125;          // two half-ulps below zl + rounding of the difference
+    const double m = 4.1 * sqrt(2.0 * ex * ex + ez * ez) + 3.0 * (2.0 * ex * ex + ez * ez) + 0.012;
+    *thr_h = (float)(ceil((4.0 + 1.25 * m) * 128.0) / 128.0);
+    *zlim = (float)zl;
+}
+
 template <int KERNEL, bool UNIFORM, bool GAMMA7>
 static cudaError_t launch_staged(sph_ctx *c)
 {
@@ -413,9 +474,11 @@ static cudaError_t launch_staged(sph_ctx *c)
     int zb = c->zblock;
     int nzb = (c->grid.nc[2] + zb - 1) / zb;
     uint64_t blocks = (uint64_t)c->grid.nc[0] * c->grid.nc[1] * nzb;
+    float thr_h, zlim;
+    filter_threshold(zb, &thr_h, &zlim);
     kern<<<(uint32_t)blocks, IA_THREADS, sizeof(IaSmem) + SPH_IA_PAD, c->stream>>>(
         c->pos4[c->cur], c->velrho4[c->cur], c->idt[c->cur], c->keyword, c->cell_begin, c->acc4, c->grid,
-        c->phys, zb, nzb);
+        c->phys, zb, nzb, thr_h, zlim);
     c->n_launches++;
     return cudaGetLastError();
 }
