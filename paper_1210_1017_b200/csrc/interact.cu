@@ -136,7 +136,7 @@ interact_simple_kernel(uint32_t n, const float4 *__restrict__ pos4, const float4
 #define SPH_IA_PAD 0          // extra dynamic shared memory per CTA (occupancy experiments)
 #endif
 #ifndef SPH_IA_DRAIN
-#define SPH_IA_DRAIN 3
+#define SPH_IA_DRAIN 4
 #endif
 #ifndef SPH_IA_QCAP
 #define SPH_IA_QCAP 11
@@ -365,25 +365,44 @@ interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict
                 }
             }
             __syncthreads();
-            // ---- stage: coalesced global reads, one column after the other
-            for (int col = 0; col < 9; ++col) {
-                const uint32_t lo = S.stage_lo[col], hi = S.stage_hi[col];
-                const int32_t off = S.stage_off[col];
-                for (uint32_t j = lo + tid; j < hi; j += IA_THREADS) {
-                    const float4 p = __ldg(pos4 + j);
-                    float4 v = __ldg(velrho4 + j);
-                    if (!UNIFORM && (__ldg(idt + j) & TYPE_BIT)) v.w = -v.w;
-                    const float xr = p.x - ox, yr = p.y - oy, zr = p.z - oz;
-                    const uint32_t si = (uint32_t)((int32_t)j + off);
-                    S.rel[si] = make_float4(xr, yr, zr, p.w);
-                    S.vr[si] = v;
-                    const float xq = (xr - ccx) * inv_h, yq = (yr - ccy) * inv_h, zq = (zr - ccz) * inv_h;
-                    if (!(fabsf(xq) < 8.0f && fabsf(yq) < 8.0f && fabsf(zq) < zlim)) s_wide = 1u;
-                    // block si / 16: x words at +0, y at +32, z at +64; candidate c = si % 16 is half c / 8 of word c % 8
-                    const uint32_t a = hp_base + 96u * (si >> 4) + 4u * (si & 7u) + ((si >> 2) & 2u);
-                    sts_u16(a, __half_as_ushort(__float2half_rn(xq)));
-                    sts_u16(a + 32u, __half_as_ushort(__float2half_rn(yq)));
-                    sts_u16(a + 64u, __half_as_ushort(__float2half_rn(zq)));
+            // ---- stage: the batch is the virtual concatenation [bstart, bend) of the 9 column ranges and
+            // smem index = virtual index - bstart.  Four candidates per thread per round with all their
+            // global loads issued before the first use, so a round costs one memory latency, not four.
+            const uint32_t nst = bend - bstart;
+            for (uint32_t k0 = tid; k0 < nst; k0 += 4u * IA_THREADS) {
+                float4 p[4], v[4];
+                bool bnd[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const uint32_t si = k0 + (uint32_t)u * IA_THREADS;
+                    bnd[u] = false;
+                    if (si < nst) {
+                        const uint32_t vv = bstart + si;
+                        int col = 0;
+#pragma unroll
+                        for (int q = 1; q < 9; ++q) col += (vv >= S.col_vstart[q]) ? 1 : 0;
+                        const uint32_t j = S.cbt[col][0] + (vv - S.col_vstart[col]);
+                        p[u] = __ldg(pos4 + j);
+                        v[u] = __ldg(velrho4 + j);
+                        if (!UNIFORM) bnd[u] = (__ldg(idt + j) & TYPE_BIT) != 0;
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const uint32_t si = k0 + (uint32_t)u * IA_THREADS;
+                    if (si < nst) {
+                        if (!UNIFORM && bnd[u]) v[u].w = -v[u].w;
+                        const float xr = p[u].x - ox, yr = p[u].y - oy, zr = p[u].z - oz;
+                        S.rel[si] = make_float4(xr, yr, zr, p[u].w);
+                        S.vr[si] = v[u];
+                        const float xq = (xr - ccx) * inv_h, yq = (yr - ccy) * inv_h, zq = (zr - ccz) * inv_h;
+                        if (!(fabsf(xq) < 8.0f && fabsf(yq) < 8.0f && fabsf(zq) < zlim)) s_wide = 1u;
+                        // block si / 16: x words at +0, y at +32, z at +64; candidate c = si % 16 is half c / 8 of word c % 8
+                        const uint32_t a = hp_base + 96u * (si >> 4) + 4u * (si & 7u) + ((si >> 2) & 2u);
+                        sts_u16(a, __half_as_ushort(__float2half_rn(xq)));
+                        sts_u16(a + 32u, __half_as_ushort(__float2half_rn(yq)));
+                        sts_u16(a + 64u, __half_as_ushort(__float2half_rn(zq)));
+                    }
                 }
             }
             __syncthreads();
