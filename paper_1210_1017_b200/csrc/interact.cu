@@ -9,12 +9,13 @@
 //    column.  With z-fastest keys the candidates of all its targets are 9 contiguous sorted
 //    ranges (one per neighbouring column); they are staged once in shared memory.  Each thread
 //    owns one target particle and works in two phases so that warps stay converged:
-//      filter - stream its 27-cell window from shared memory (broadcast reads), 6 flops + a
-//               compare per candidate, push the smem index of every candidate inside 2h on a
-//               private shared-memory stack;
-//      drain  - whenever a stack in the warp is nearly full (and at the end) all lanes pop one
-//               entry and evaluate the full pair term, so the expensive path runs with (almost)
-//               all lanes active instead of the ~14 % a fused test+interact loop would have.
+//      filter - stream its 27-cell window from an fp16 copy of the staged positions (broadcast
+//               reads, two candidates per half2 instruction, conservative threshold), push the hit
+//               mask of every block of 16 candidates on a private shared-memory stack;
+//      drain  - whenever a stack in the warp is full (and at the end) all lanes pop pending entries
+//               and evaluate the full pair term in fp32 from the exact records, so the expensive
+//               path runs with (almost) all lanes active instead of the ~14 % a fused
+//               test+interact loop would have.
 //  * interact_simple_kernel (cross-check, SPH_OPT_INTERACT_VARIANT = 1): one thread per
 //    particle walking the cell table with global loads, as the paper describes it.
 //

@@ -102,6 +102,38 @@ def test_dense_cells_use_several_batches_and_chunks():
     assert e_d <= TOL_RATE and e_a <= TOL_RATE
 
 
+def test_particles_outside_the_grid_widen_the_fp16_filter():
+    """Reading A13: particles beyond the grid sit clamped in edge cells.  The interaction kernel's
+    fp16 filter is derived for particles inside their cells; a CTA that meets one outside that
+    model must let every candidate through to the exact fp32 evaluation.  Here the grid stops at a
+    third of the tank in x, so the far wall and part of the floor are up to ~17 h outside."""
+    w = W.dam_break(12, scrambled=True)
+    P = dict(w.params)
+    P["dom_max"] = (W.f32(P["dom_min"][0] + 10.0 * 2.0 * P["h"]), P["dom_max"][1], P["dom_max"][2])
+    w.params = P
+    assert (w.pos[:, 0] > P["dom_max"][0] + 8.0 * P["h"]).any()
+    ref_a, ref_d = oracle_rates(w)
+    out = _gpu_rates(w, 0)
+    e_d, e_a = rate_errors(w, out["acc"], out["drho"], ref_a, ref_d)
+    assert e_d <= TOL_RATE and e_a <= TOL_RATE
+
+
+def test_sparse_cells_long_z_blocks():
+    """h = 0.75 dp: 3.4 particles per cell, so a CTA owns the maximum run of 32 cells and the fp16
+    filter works with its widest z range (|z| < 64 h) and largest error pad."""
+    w = W.dam_break(16, scrambled=True)
+    P = dict(w.params)
+    P["h"] = W.f32(0.75 * P["dp"])
+    w.params = P
+    ref_a, ref_d = oracle_rates(w)
+    assert np.abs(ref_d).max() > 0
+    out = _gpu_rates(w, 0)
+    e_d, e_a = rate_errors(w, out["acc"], out["drho"], ref_a, ref_d)
+    assert e_d <= TOL_RATE and e_a <= TOL_RATE
+    b = _gpu_rates(w, 1)
+    assert np.abs(out["drho"] - b["drho"]).max() <= 2e-5 * np.abs(b["drho"]).max()
+
+
 def _run_ten_steps(w, steps=10):
     sph = make_sph(w)
     nc = OA.grid_dims(w.params["dom_min"], w.params["dom_max"], w.params["h"])
