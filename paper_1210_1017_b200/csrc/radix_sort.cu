@@ -51,7 +51,6 @@ struct __align__(16) RsSmem {
     uint2 stage[RS_TILE];                 // 64 KB
     uint2 wm[RS_WARPS][256];              // 16 KB: per warp and digit, .x = match mask of the row being
                                           // ranked (scratch, 0 between rows), .y = running count
-    uint32_t digit_start[256];            // first tile-local slot of each digit
     uint32_t gbase[256];                  // global slot of tile-local slot 0 of each digit
     uint32_t scan_tmp[16];
     uint32_t tile;
@@ -154,8 +153,10 @@ __device__ __forceinline__ void onesweep_tile(RsSmem &S, uint32_t n, const uint2
             hadd += (w < (int)warp) ? S.scan_tmp[8 + w] : 0u;
         }
         dstart += exc_in_warp;
-        S.digit_start[tid] = dstart;
         S.gbase[tid] = hexc_in_warp + hadd - dstart;    // + look-back, added below
+        // fold the digit's first slot into the per-warp bases: one look-up per pair in the reorder
+#pragma unroll
+        for (int w = 0; w < RS_WARPS; ++w) S.wm[w][tid].y += dstart;
     }
     __syncthreads();
 
@@ -164,7 +165,7 @@ __device__ __forceinline__ void onesweep_tile(RsSmem &S, uint32_t n, const uint2
     for (int k = 0; k < RS_IPT; ++k) {
         const uint32_t d = (kv[k].x >> shift) & dmask;
         const uint32_t r = (k & 1) ? (rank2[k >> 1] >> 16) : (rank2[k >> 1] & 0xFFFFu);
-        S.stage[S.digit_start[d] + wm_warp[d].y + r] = kv[k];
+        S.stage[wm_warp[d].y + r] = kv[k];
     }
 
     // ---- finish the look-back: same digit in earlier tiles, RS_LB polls per round
