@@ -143,11 +143,17 @@ interact_simple_kernel(uint32_t n, const float4 *__restrict__ pos4, const float4
 #define SPH_IA_QCAP 11
 #endif
 constexpr int IA_DRAIN = SPH_IA_DRAIN;   // pairs a lane evaluates per drain round
-constexpr int IA_THREADS = 256;
+#ifndef SPH_IA_THREADS
+#define SPH_IA_THREADS 256
+#endif
+#ifndef SPH_IA_CAP
+#define SPH_IA_CAP 2688
+#endif
+constexpr int IA_THREADS = SPH_IA_THREADS;
 constexpr int IA_QCAP = SPH_IA_QCAP; // stack entries per thread; one entry = hit mask of one block of IA_BLK candidates
 constexpr int IA_BLK = 16;           // candidates per filter block = per stack entry
 constexpr int IA_ZMAX = 32;          // max cells per z-block
-constexpr int IA_CAP = 2688;         // staged candidates per batch (9 columns x 11 cells x 27 + slack), multiple of 16
+constexpr int IA_CAP = SPH_IA_CAP;   // staged candidates per batch (9 columns x 11 cells x 27 + slack), multiple of 16
 constexpr int IA_NBLK = IA_CAP / IA_BLK;
 constexpr float IA_TINY = 1e-30f;    // r2 floor: a coincident pair (the particle itself) adds exactly 0
 static_assert(IA_CAP % IA_BLK == 0 && IA_NBLK <= 256, "block index must fit 8 bits of a stack entry");
@@ -170,6 +176,7 @@ struct IaSmem {
 };
 
 size_t interact_smem_bytes(const sph_ctx *) { return sizeof(IaSmem); }
+int interact_threads() { return IA_THREADS; }
 
 __device__ __forceinline__ void sts_u32(uint32_t addr, uint32_t v)
 {

@@ -288,9 +288,9 @@ int sph_init(sph_ctx **out, const sph_params *p, const sph_particles *part, int 
     c->prev_init = (uint8_t *)(w + L.prev_init);
     c->flags = (uint32_t *)(w + L.flags);
     c->interact_variant = 0;
-    // cells per z-block of the interaction kernel: fill the 256-thread CTA with targets
+    // cells per z-block of the interaction kernel: fill the CTA's threads with targets
     double ppc = pow(2.0 * (double)p->h / (double)p->dp, 3.0);
-    int zb = (int)floor(256.0 * 0.97 / (ppc > 0.05 ? ppc : 0.05));
+    int zb = (int)floor((double)interact_threads() * 0.97 / (ppc > 0.05 ? ppc : 0.05));
     if (zb < 1) zb = 1;
     if (zb > 32) zb = 32;
     c->zblock = zb;

@@ -139,6 +139,7 @@ uint32_t gather_tiles(uint64_t n);
 uint32_t mig_groups(uint64_t n);
 size_t gap_list_entries(uint64_t ncells);
 size_t interact_smem_bytes(const sph_ctx *c);
+int interact_threads();
 
 // Tait pressure over rho^2 from rho, fp32, cancellation-free.
 __device__ __forceinline__ float tait_p_over_rho2(float rho, const PhysC &ph)
