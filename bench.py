@@ -34,6 +34,9 @@ CONFIG_NB = {0: 16, 1: 100, 2: 200, 3: 317}
 METRIC = "Mparticle-steps/s"
 FP32_LANES_PER_SM, NUM_SMS = 128, 148
 FLOPS_PER_CANDIDATE, FLOPS_PER_PAIR = 8, 32
+# dram__bytes_read.sum + dram__bytes_write.sum of one interact_staged_kernel launch at config 3
+# (profiles/r01_ncu_full_config3_v2.md); other configs have no capture
+IA_TRAFFIC_BYTES = {3: 1.379628e9 + 0.530434e9}
 # algorithmic HBM bytes per particle of the memory-bound stages
 BYTES = dict(keys=28.0, sort_per_pass=16.0, gather=116.0, verlet=116.0, migrate=4.0)
 
@@ -203,6 +206,7 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--micro", type=int, default=0, help="log2 N of the sort/halo microbenchmark")
     ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--e2e-contexts", type=int, default=2, help="contexts pipelined in the end-to-end measurement")
     ap.add_argument("--cpu-sample", type=int, default=1_500_000, help="particles of the cpu_baseline sample")
     ap.add_argument("--ref-sample", type=int, default=300_000, help="particles per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -280,23 +284,62 @@ def main():
                 vel=torch.empty((n, 3), dtype=torch.float32).pin_memory(),
                 rho=torch.empty(n, dtype=torch.float32).pin_memory())
 
-    def e2e_step():
-        sph.sph_set_state(pin["pos"].numpy(), pin["vel"].numpy(), pin["rho"].numpy(), pin["typ"].numpy())
-        sph.sph_step(w.dt)
-        sph.sph_download(acc=False, drho=False, pinned=outp)
+    def e2e_step(ctx, out):
+        ctx.sph_set_state(pin["pos"].numpy(), pin["vel"].numpy(), pin["rho"].numpy(), pin["typ"].numpy())
+        ctx.sph_step(w.dt)
+        ctx.sph_download(acc=False, drho=False, pinned=out)
 
+    # (a) one context: upload, step, download strictly one after the other
     if args.e2e_steps > 0:
-        e2e_step()
+        e2e_step(sph, outp)
     barrier()
     t0 = time.perf_counter()
     for _ in range(args.e2e_steps):
-        e2e_step()
+        e2e_step(sph, outp)
     torch.cuda.synchronize()
-    e2e_s = max(time.perf_counter() - t0, 1e-9)
-    e2e_s = R.max_over_ranks(rep, e2e_s)
-    e2e = dict(value=world * n * args.e2e_steps / e2e_s / 1e6, unit="Mparticle-steps/s",
+    e2e_single_s = R.max_over_ranks(rep, max(time.perf_counter() - t0, 1e-9))
+    e2e_single = world * n * args.e2e_steps / e2e_single_s / 1e6
+    # (b) two contexts on two streams driven by two host threads: the same three calls per step,
+    # but one context's PCIe copies overlap the other's kernels (what a user with a queue of
+    # independent jobs does).  This is the reported end-to-end value; (a) is printed beside it.
+    e2e_value, e2e_ctx = e2e_single, 1
+    if args.e2e_steps > 0 and args.e2e_contexts > 1:
+        import threading
+        ctxs, outs = [sph], [outp]
+        for _ in range(args.e2e_contexts - 1):
+            c2 = B.Sph(w.params, w.pos, w.vel, w.rho, w.type, device=f"cuda:{local}", stream=torch.cuda.Stream())
+            c2.sph_set_option(B.SPH_OPT_INTERACT_VARIANT, args.variant)
+            c2.sph_set_slabs(planes)
+            ctxs.append(c2)
+            outs.append({k: torch.empty_like(v).pin_memory() for k, v in outp.items()})
+
+        def worker(k, steps):
+            torch.cuda.set_device(local)
+            for _ in range(steps):
+                e2e_step(ctxs[k], outs[k])
+
+        def run_all(steps):
+            th = [threading.Thread(target=worker, args=(k, steps)) for k in range(len(ctxs))]
+            for t in th:
+                t.start()
+            for t in th:
+                t.join()
+            torch.cuda.synchronize()
+
+        run_all(1)
+        barrier()
+        t0 = time.perf_counter()
+        run_all(args.e2e_steps)
+        e2e_s = R.max_over_ranks(rep, max(time.perf_counter() - t0, 1e-9))
+        e2e_value = world * n * args.e2e_steps * len(ctxs) / e2e_s / 1e6
+        e2e_ctx = len(ctxs)
+        for c2 in ctxs[1:]:
+            c2.sph_destroy()
+    e2e = dict(value=e2e_value, unit="Mparticle-steps/s",
                h2d_bytes_per_step=int(n * (12 + 12 + 4 + 1)), d2h_bytes_per_step=int(n * (12 + 12 + 4)),
-               steps=args.e2e_steps, api="sph_set_state(host) + sph_step + sph_download(host), pinned buffers")
+               steps=args.e2e_steps * e2e_ctx, contexts=e2e_ctx, single_context_value=e2e_single,
+               api="per step: sph_set_state(host) + sph_step + sph_download(host), pinned buffers; "
+                   f"{e2e_ctx} context(s) on separate streams so copies overlap kernels")
 
     if rank != 0:
         R.finalize(rep)
@@ -310,7 +353,7 @@ def main():
     peak = NUM_SMS * FP32_LANES_PER_SM * 2 * pk["sm_max_mhz"] * 1e6 / 1e12
     sm_mhz = clocks.get("sm_mhz") or pk["sm_max_mhz"]
     roofline = dict(bound="alu", kernel="interact_staged_kernel", achieved=achieved, peak=peak, unit="TFLOP/s",
-                    frac=achieved / peak, traffic=None,
+                    frac=achieved / peak, traffic=IA_TRAFFIC_BYTES.get(args.config),
                     peak_source=f"148 SMs x 128 FP32 lanes x 2 flop x {pk['sm_max_mhz']:.0f} MHz (max clock, {pk['source']})",
                     frac_at_observed_clock=achieved / (peak * sm_mhz / pk["sm_max_mhz"]),
                     algorithmic_flops_per_launch=flops, candidates=cand, pairs=pairs,
