@@ -29,6 +29,7 @@ constexpr int RS_THREADS = SPH_RS_THREADS;        // >= 256 (one thread per digi
 constexpr int RS_IPT = SPH_RS_IPT;                // pairs per thread (even)
 constexpr int RS_TILE = RS_THREADS * RS_IPT;      // 8192 pairs = 64 KB staged
 constexpr int RS_WARPS = RS_THREADS / 32;
+constexpr int RS_UNITS = RS_THREADS / 16;         // ranking units: half-warps (16-bit masks, 32-bit table entries)
 constexpr int RS_LB = 8;                          // look-back polls in flight per thread
 constexpr uint32_t LB_AGG = 1u << 30;             // look-back word: flag in bits 30..31
 constexpr uint32_t LB_INC = 2u << 30;
@@ -49,33 +50,35 @@ __device__ __forceinline__ void st_relaxed(uint32_t *p, uint32_t v)
 
 struct __align__(16) RsSmem {
     uint2 stage[RS_TILE];                 // 64 KB
-    uint2 wm[RS_WARPS][256];              // 16 KB: per warp and digit, .x = match mask of the row being
-                                          // ranked (scratch, 0 between rows), .y = running count
+    uint32_t hw[RS_UNITS][256];           // 16 KB: per half-warp and digit, low 16 bits = match mask of the row
+                                          // being ranked (scratch, 0 between rows), high 16 = running count
     uint32_t gbase[256];                  // global slot of tile-local slot 0 of each digit
     uint32_t scan_tmp[16];
     uint32_t tile;
 };
 
-// Stable warp-level ranking of one row (32 items, one per lane) on an 8-bit digit.  The set of
-// lanes holding the same digit is built in shared memory: every lane ORs its lane bit into the
-// (warp, digit) mask word - OR commutes, so the result does not depend on the order in which the
-// hardware serialises lanes that hit the same word - and reads the word back together with the
-// running count of that digit in earlier rows of the warp.  One ATOMS + one LDS.64 + one STS.64
-// replace the eight ballots (about 50 ALU-pipe instructions) of a register-only match.
-__device__ __forceinline__ uint32_t rank_row(uint32_t wm_warp /* shared address of S.wm[warp] */, uint32_t d,
-                                             uint32_t lane_bit, uint32_t lt_mask)
+// Stable ranking of one row of a half-warp (16 items, one per lane) on an 8-bit digit.  The set of
+// lanes holding the same digit is built in shared memory: every lane ORs its bit into the (unit, digit)
+// word - OR commutes, so the result does not depend on the order in which the hardware serialises
+// lanes that hit the same word - and reads the word back: low half = the set, high half = the running
+// count of that digit in earlier rows of the unit.  One ATOMS + one LDS + one STS, all 32-bit (random
+// digits spread over all 32 banks), replace the eight ballots (about 50 ALU-pipe instructions) of a
+// register-only match.  Both half-warps of a warp work on their own tables in the same instructions.
+__device__ __forceinline__ uint32_t rank_row(uint32_t table /* shared address of S.hw[unit] */, uint32_t d,
+                                             uint32_t bit16, uint32_t lt16)
 {
-    const uint32_t e = wm_warp + 8u * d;
-    uint32_t mx, my;
-    asm volatile("red.shared.or.b32 [%0], %1;" ::"r"(e), "r"(lane_bit) : "memory");
+    const uint32_t e = table + 4u * d;
+    uint32_t w;
+    asm volatile("red.shared.or.b32 [%0], %1;" ::"r"(e), "r"(bit16) : "memory");
     __syncwarp();
-    asm volatile("ld.shared.v2.u32 {%0,%1}, [%2];" : "=r"(mx), "=r"(my) : "r"(e) : "memory");
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(w) : "r"(e) : "memory");
     __syncwarp();
-    const uint32_t below = mx & lt_mask;
+    const uint32_t m = w & 0xFFFFu, cnt = w >> 16;
+    const uint32_t below = m & lt16;
     if (below == 0)                                                    // lowest lane of the set
-        asm volatile("st.shared.v2.u32 [%0], {%1,%2};" ::"r"(e), "r"(0u), "r"(my + __popc(mx)) : "memory");
+        asm volatile("st.shared.u32 [%0], %1;" ::"r"(e), "r"((cnt + __popc(m)) << 16) : "memory");
     __syncwarp();
-    return my + __popc(below);
+    return cnt + __popc(below);
 }
 
 template <bool FULL>
@@ -84,29 +87,31 @@ __device__ __forceinline__ void onesweep_tile(RsSmem &S, uint32_t n, const uint2
                                               uint32_t *tile_state, int shift, uint32_t dmask, uint32_t tile)
 {
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const uint32_t lane_bit = 1u << lane, lt_mask = lane_bit - 1u;
+    const uint32_t unit = tid >> 4, lane16 = tid & 15u;
+    const uint32_t bit16 = 1u << lane16, lt16 = bit16 - 1u;
     const uint32_t base = tile * RS_TILE;
     const uint32_t tile_n = FULL ? (uint32_t)RS_TILE : n - base;
 
-    // ---- load, warp-striped: the warp owns a contiguous chunk; item k of lane l is chunk[k*32+l].
+    // ---- load, striped per half-warp: the unit owns a contiguous chunk; item k of its lane l is
+    // chunk[k*16+l], so that (unit, row, lane) order is index order.
     // Slots past the end of the array hold the key 0xFFFFFFFF: its digit is dmask, the largest digit
     // of the pass, and a stable ranking puts those slots after every real pair of the tile, i.e. at
     // staged positions >= tile_n, which are never written out.
     uint2 kv[RS_IPT];
-    const uint32_t wbase = warp * (32 * RS_IPT);
+    const uint32_t ubase = unit * (16 * RS_IPT);
 #pragma unroll
     for (int k = 0; k < RS_IPT; ++k) {
-        const uint32_t li = wbase + k * 32 + lane;
+        const uint32_t li = ubase + k * 16 + lane16;
         kv[k] = (FULL || li < tile_n) ? __ldcs(in + base + li) : make_uint2(0xFFFFFFFFu, 0u);
     }
     // ---- rank inside the warp, stable in item order; two 16-bit ranks per register
     uint32_t rank2[RS_IPT / 2];
-    const uint32_t wm_addr = (uint32_t)__cvta_generic_to_shared(S.wm[warp]);
-    const uint2 *wm_warp = S.wm[warp];
+    const uint32_t tab_addr = (uint32_t)__cvta_generic_to_shared(S.hw[unit]);
+    const uint32_t *tab = S.hw[unit];
 #pragma unroll
     for (int k = 0; k < RS_IPT; ++k) {
         const uint32_t d = (kv[k].x >> shift) & dmask;
-        const uint32_t r = rank_row(wm_addr, d, lane_bit, lt_mask);
+        const uint32_t r = rank_row(tab_addr, d, bit16, lt16);
         if (k & 1) rank2[k >> 1] |= r << 16; else rank2[k >> 1] = r;
     }
     __syncthreads();
@@ -119,9 +124,9 @@ __device__ __forceinline__ void onesweep_tile(RsSmem &S, uint32_t n, const uint2
     uint32_t *st = tile_state + (size_t)tile * 256 + (tid & 255);
     if (tid < 256) {
 #pragma unroll
-        for (int w = 0; w < RS_WARPS; ++w) {
-            const uint32_t t = S.wm[w][tid].y;
-            S.wm[w][tid].y = count;
+        for (int u = 0; u < RS_UNITS; ++u) {
+            const uint32_t t = S.hw[u][tid] >> 16;
+            S.hw[u][tid] = count;                                   // from here on: plain 32-bit bases
             count += t;
         }
         const uint32_t pads = FULL ? 0u : (tid == dmask ? (uint32_t)RS_TILE - tile_n : 0u);
@@ -156,7 +161,7 @@ __device__ __forceinline__ void onesweep_tile(RsSmem &S, uint32_t n, const uint2
         S.gbase[tid] = hexc_in_warp + hadd - dstart;    // + look-back, added below
         // fold the digit's first slot into the per-warp bases: one look-up per pair in the reorder
 #pragma unroll
-        for (int w = 0; w < RS_WARPS; ++w) S.wm[w][tid].y += dstart;
+        for (int u = 0; u < RS_UNITS; ++u) S.hw[u][tid] += dstart;
     }
     __syncthreads();
 
@@ -165,7 +170,7 @@ __device__ __forceinline__ void onesweep_tile(RsSmem &S, uint32_t n, const uint2
     for (int k = 0; k < RS_IPT; ++k) {
         const uint32_t d = (kv[k].x >> shift) & dmask;
         const uint32_t r = (k & 1) ? (rank2[k >> 1] >> 16) : (rank2[k >> 1] & 0xFFFFu);
-        S.stage[wm_warp[d].y + r] = kv[k];
+        S.stage[tab[d] + r] = kv[k];
     }
 
     // ---- finish the look-back: same digit in earlier tiles, RS_LB polls per round
@@ -218,8 +223,8 @@ onesweep_kernel(uint32_t n, const uint2 *__restrict__ in, uint2 *__restrict__ ou
     const uint32_t tid = threadIdx.x;
     if (tid == 0) S.tile = atomicAdd(tile_counter, 1u);
     {
-        uint4 *z = reinterpret_cast<uint4 *>(&S.wm[0][0]);
-        for (int k = tid; k < RS_WARPS * 256 / 2; k += RS_THREADS) z[k] = make_uint4(0u, 0u, 0u, 0u);
+        uint4 *z = reinterpret_cast<uint4 *>(&S.hw[0][0]);
+        for (int k = tid; k < RS_UNITS * 256 / 4; k += RS_THREADS) z[k] = make_uint4(0u, 0u, 0u, 0u);
     }
     __syncthreads();
     const uint32_t tile = S.tile;
