@@ -57,6 +57,9 @@ def lib():
         L.orc_step.restype = C.c_int
         L.orc_step.argtypes = [C.POINTER(OrcParams), C.c_long, dp, dp, dp, dp, dp, C.c_void_p,
                                C.c_double, C.c_long, C.c_int, C.c_int, dp, dp]
+        L.orc_time_step.restype = C.c_int
+        L.orc_time_step.argtypes = [C.POINTER(OrcParams), C.c_long, dp, dp, dp, C.c_void_p, dp, C.c_double,
+                                    C.c_double, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, dp]
         L.orc_neighbour_pairs.restype = C.c_int
         L.orc_neighbour_pairs.argtypes = [C.POINTER(OrcParams), C.c_long, dp, C.c_long,
                                           C.POINTER(C.c_long), C.POINTER(C.c_long)]
@@ -129,6 +132,29 @@ def rates(p: OrcParams, r, v, rho, typ, p_override=None, mode=1):
                          drho.ctypes.data_as(C.POINTER(C.c_double)))
     assert rc == 0
     return acc, drho
+
+
+def time_step(p: OrcParams, r, v, rho, typ, acc, cfl=0.2, cut=1.0, slab_of=None, n_slabs=0):
+    """Variable time step of reading A8b: dict(dt, dt_f, dt_cv, mu (n,), amax_slab, smax_slab)."""
+    r, rp = _d(r)
+    v, vp = _d(v)
+    rho, rhop = _d(rho)
+    acc, ap = _d(acc)
+    typ = np.ascontiguousarray(typ, dtype=np.uint8)
+    n = rho.shape[0]
+    mu = np.zeros(n, dtype=np.float64)
+    out = np.zeros(3, dtype=np.float64)
+    am = np.zeros(max(n_slabs, 1), dtype=np.float64)
+    sm = np.zeros(max(n_slabs, 1), dtype=np.float64)
+    so = None
+    if slab_of is not None:
+        sov = np.ascontiguousarray(slab_of, dtype=np.int64)
+        so = sov.ctypes.data
+    rc = lib().orc_time_step(C.byref(p), n, rp, vp, rhop, typ.ctypes.data, ap, float(cfl), float(cut), so,
+                             int(n_slabs), am.ctypes.data, sm.ctypes.data, mu.ctypes.data,
+                             out.ctypes.data_as(C.POINTER(C.c_double)))
+    assert rc == 0
+    return dict(dt=out[0], dt_f=out[1], dt_cv=out[2], mu=mu, amax_slab=am[:n_slabs], smax_slab=sm[:n_slabs])
 
 
 class State:

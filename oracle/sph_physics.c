@@ -277,6 +277,73 @@ int orc_rates(const orc_params *P, long n, const double *r, const double *v, con
     return 0;
 }
 
+/* Variable time step (L150: "The size of the integration time step varies throughout each
+ * simulation according to the Courant-Friedrichs-Lewy (CFL) condition [20] and the magnitude of
+ * the interactions.  Here, minimum and maximum values of certain physical quantities need to be
+ * found among all particles"; L222: every sub-domain k determines its own dt_k, the step uses the
+ * minimum).  The paper gives no formula; reading A8b takes the usual pair of limits,
+ *     dt_f  = sqrt(h / max_i |a_i|)                    over fluid particles   ("magnitude of the interactions")
+ *     dt_cv = h / max_i (c_i + max_j |mu_ij|)          over all particles     (CFL with the viscous signal speed)
+ *     dt    = cfl * min(dt_f, dt_cv),
+ * mu_ij = h v_ij.r_ij / (r_ij^2 + eta^2) as in L112, j over the neighbours 0 < r_ij < cut * 2h.
+ * |mu_ij| does not vanish at the edge of the support, so max_j is discontinuous in the cut-off:
+ * `cut` (1 for the definition) lets a test bracket an fp32 implementation between cut = 1 -+ eps.
+ * Brute force O(N^2).  slab_of: NULL, or the owning sub-domain of every particle; then
+ * amax_slab / smax_slab (n_slabs each) receive the per-sub-domain maxima of |a| and c + mu.
+ * mu_out: NULL or n (max_j |mu_ij| per particle). */
+int orc_time_step(const orc_params *P, long n, const double *r, const double *v, const double *rho,
+                  const unsigned char *type, const double *acc, double cfl, double cut,
+                  const long *slab_of, int n_slabs, double *amax_slab, double *smax_slab,
+                  double *mu_out, double *dt_out /* dt, dt_f, dt_cv */)
+{
+    if (!P || n < 0 || !dt_out) return -1;
+    double h = P->h, eta2 = 0.01 * h * h, rc2 = 4.0 * h * h * cut * cut;
+    double *mu = (double *)calloc(n > 0 ? n : 1, sizeof(double));
+    if (!mu) return -1;
+#pragma omp parallel for schedule(static)
+    for (long i = 0; i < n; ++i) {
+        double m = 0.0;
+        for (long j = 0; j < n; ++j) {
+            if (j == i) continue;
+            double d[3];
+            rij_of(P, r + 3 * i, r + 3 * j, d);
+            double r2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+            if (!(r2 < rc2) || !(r2 > 0.0)) continue;
+            double dot = (v[3 * i] - v[3 * j]) * d[0] + (v[3 * i + 1] - v[3 * j + 1]) * d[1] +
+                         (v[3 * i + 2] - v[3 * j + 2]) * d[2];
+            double a = fabs(h * dot / (r2 + eta2));
+            if (a > m) m = a;
+        }
+        mu[i] = m;
+    }
+    double amax = 0.0, smax = 0.0;
+    for (int k = 0; k < n_slabs; ++k) { if (amax_slab) amax_slab[k] = 0.0; if (smax_slab) smax_slab[k] = 0.0; }
+    for (long i = 0; i < n; ++i) {
+        double s = orc_sound_speed(P, rho[i]) + mu[i];
+        if (s > smax) smax = s;
+        double a = 0.0;
+        if (!type || type[i] == 0) {
+            a = sqrt(acc[3 * i] * acc[3 * i] + acc[3 * i + 1] * acc[3 * i + 1] + acc[3 * i + 2] * acc[3 * i + 2]);
+            if (a > amax) amax = a;
+        }
+        if (slab_of && n_slabs > 0) {
+            long k = slab_of[i];
+            if (k >= 0 && k < n_slabs) {
+                if (smax_slab && s > smax_slab[k]) smax_slab[k] = s;
+                if (amax_slab && a > amax_slab[k]) amax_slab[k] = a;
+            }
+        }
+        if (mu_out) mu_out[i] = mu[i];
+    }
+    free(mu);
+    double dt_f = amax > 0.0 ? sqrt(h / amax) : INFINITY;
+    double dt_cv = smax > 0.0 ? h / smax : INFINITY;
+    dt_out[1] = dt_f;
+    dt_out[2] = dt_cv;
+    dt_out[0] = cfl * (dt_f < dt_cv ? dt_f : dt_cv);
+    return 0;
+}
+
 /* Number of neighbours (0 < r < 2h) of each particle by brute force; used by structure
  * pins (halo sufficiency).  nbr_count: n. */
 int orc_neighbour_pairs(const orc_params *P, long n, const double *r, long max_pairs,

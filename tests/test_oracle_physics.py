@@ -299,3 +299,73 @@ def test_hydrostatic_column_bottom_pressure():
     # the column stays a column (no lateral drift, little vertical motion)
     assert np.abs(s.r[typ == 0, :2] - rf[:, :2]).max() < 0.05 * dp
     assert np.abs(s.r[typ == 0, 2] - rf[:, 2]).max() < 0.5 * dp
+
+
+# ---- variable time step (reading A8b; L150, L222) ---------------------------------------------
+def test_time_step_two_particles_by_hand():
+    """h = 0.1, eta^2 = 0.01 h^2 = 1e-4.  Particles 0.15 apart along x approaching at 1 m/s:
+    mu = h |v.r| / (r^2 + eta^2) = 0.1 * 0.15 / (0.0225 + 0.0001) = 0.015 / 0.0226.
+    dt_cv = h / (c0 + mu) with rho = rho0; dt_f = sqrt(h / 9.81) from the larger acceleration."""
+    p = OB.make_params(h=0.1, c0=10.0)
+    r = np.array([[0, 0, 0], [0.15, 0, 0.0]])
+    v = np.array([[0, 0, 0], [-1.0, 0, 0]])
+    rho = np.array([1000.0, 1000.0])
+    acc = np.array([[0, 0, -9.81], [0, 0, -2.0]])
+    o = OB.time_step(p, r, v, rho, np.zeros(2, np.uint8), acc, cfl=0.2)
+    mu = 0.015 / 0.0226
+    assert np.allclose(o["mu"], [mu, mu], rtol=1e-14)
+    assert abs(o["dt_cv"] - 0.1 / (10.0 + mu)) < 1e-16
+    assert abs(o["dt_f"] - np.sqrt(0.1 / 9.81)) < 1e-16
+    assert abs(o["dt"] - 0.2 * 0.1 / (10.0 + mu)) < 1e-16
+    # receding pairs count with their magnitude too (|mu|)
+    o2 = OB.time_step(p, r, -v, rho, np.zeros(2, np.uint8), acc, cfl=0.2)
+    assert np.allclose(o2["mu"], o["mu"], rtol=1e-14)
+    # a boundary particle's acceleration does not limit the step; beyond 2h there is no pair
+    o3 = OB.time_step(p, r * 2.0, v, rho, np.array([1, 0], np.uint8), acc, cfl=0.2)
+    assert (o3["mu"] == 0).all() and abs(o3["dt_f"] - np.sqrt(0.1 / 2.0)) < 1e-16
+    assert abs(o3["dt_cv"] - 0.1 / 10.0) < 1e-18
+
+
+def test_time_step_uniform_expansion_on_a_lattice_and_the_cut_off():
+    """dp = 1, h = 1.5 (4h^2 = 9 exactly), v = A r: v_ij.r_ij = A r^2, so mu grows with r and the
+    maximum sits at the farthest neighbour: |n|^2 = 8 inside the support, the 30 lattice points at
+    |n|^2 = 9 lie exactly ON the edge (excluded by r < 2h, included by cut > 1): this is the
+    discontinuity a bracketing comparison of an fp32 implementation has to allow for."""
+    n1 = 7
+    g = np.arange(n1, dtype=np.float64)
+    r = np.stack(np.meshgrid(g, g, g, indexing="ij"), -1).reshape(-1, 3)
+    A = 0.3
+    v = A * r
+    rho = np.full(len(r), 1000.0)
+    p = OB.make_params(h=1.5, c0=20.0)
+    acc = np.zeros_like(r)
+    centre = (3 * n1 + 3) * n1 + 3
+    o = OB.time_step(p, r, v, rho, np.zeros(len(r), np.uint8), acc)
+    assert abs(o["mu"][centre] - 1.5 * A * 8.0 / (8.0 + 0.0225)) < 1e-14
+    o = OB.time_step(p, r, v, rho, np.zeros(len(r), np.uint8), acc, cut=1.0 + 1e-9)
+    assert abs(o["mu"][centre] - 1.5 * A * 9.0 / (9.0 + 0.0225)) < 1e-14
+    assert o["dt_f"] == np.inf
+
+
+def test_time_step_per_slab_minimum_is_the_global_one():
+    """L222: every sub-domain finds its own dt_k; the step uses the minimum."""
+    rng = np.random.default_rng(5)
+    n = 400
+    r = rng.random((n, 3)) * 0.5
+    v = rng.normal(size=(n, 3))
+    rho = 1000.0 * (1 + 0.01 * rng.random(n))
+    typ = (rng.random(n) < 0.2).astype(np.uint8)
+    acc = rng.normal(size=(n, 3)) * 10
+    p = OB.make_params(h=0.05, c0=30.0)
+    slab = np.minimum((r[:, 0] / 0.5 * 4).astype(np.int64), 3)
+    o = OB.time_step(p, r, v, rho, typ, acc, cfl=0.2, slab_of=slab, n_slabs=4)
+    dt_k = 0.2 * np.minimum(np.sqrt(0.05 / o["amax_slab"]), 0.05 / o["smax_slab"])
+    assert abs(dt_k.min() - o["dt"]) < 1e-18
+    # brute-force restatement of the maxima in numpy
+    fl = typ == 0
+    assert abs(o["amax_slab"].max() - np.linalg.norm(acc[fl], axis=1).max()) < 1e-12
+    d = r[:, None, :] - r[None, :, :]
+    r2 = (d ** 2).sum(-1)
+    dot = ((v[:, None, :] - v[None, :, :]) * d).sum(-1)
+    mu = np.where((r2 < 4 * 0.05 ** 2) & (r2 > 0), np.abs(0.05 * dot / (r2 + 0.01 * 0.05 ** 2)), 0.0).max(1)
+    assert np.allclose(mu, o["mu"], rtol=1e-12, atol=0)
