@@ -211,6 +211,7 @@ def main():
     ap.add_argument("--ref-sample", type=int, default=300_000, help="particles per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--variant", type=int, default=0)
+    ap.add_argument("--adaptive", action="store_true", help="timed steps use sph_step_adaptive(cfl = 0.2) (variable dt)")
     args = ap.parse_args()
     if args.steps is None:
         args.steps = 10 if (args.impl == "reference" or args.micro) else {0: 200, 1: 200, 2: 200, 3: 100}[args.config]
@@ -265,7 +266,10 @@ def main():
     sampler.start()
     ev0.record()
     for _ in range(args.steps):
-        sph.sph_step(w.dt)
+        if args.adaptive:
+            sph.sph_step_adaptive(0.2)
+        else:
+            sph.sph_step(w.dt)
     ev1.record()
     barrier()
     clocks = sampler.stop()
@@ -390,7 +394,7 @@ def main():
         config=dict(workload=f"config{args.config}: 3-D dam break, {w.n_fluid} fluid + {n - w.n_fluid} boundary "
                              f"particles, {w.n_slabs} logical x-slabs",
                     n_particles=n, n_slabs=w.n_slabs, cells=int(v.ncells), cell_bits=int(v.cell_bits),
-                    radix_passes=passes, dt=w.dt, multi_gpu="replicas only",
+                    radix_passes=passes, dt=("variable, cfl 0.2" if args.adaptive else w.dt), multi_gpu="replicas only",
                     l2="no flush: per-step working set %.1f GB >> 126 MB L2" % (n * 250e-9)
                     if n > 5_000_000 else "working set fits L2 (small config)"),
         clocks=clocks, e2e=e2e, gpu_launches=int(launches), roofline=roofline, cpu_baseline=cpu,

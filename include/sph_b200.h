@@ -119,8 +119,11 @@ enum {
 
 /* Options for sph_set_option. */
 enum {
-    SPH_OPT_INTERACT_VARIANT = 0  /* 0 = smem-staged production kernel, 1 = simple
+    SPH_OPT_INTERACT_VARIANT = 0, /* 0 = smem-staged production kernel, 1 = simple
                                      one-thread-per-particle kernel (cross-check) */
+    SPH_OPT_ADAPTIVE_DT = 1       /* 1 = sph_interact also records max_j |mu_ij| of every particle,
+                                     which sph_time_step needs (costs a few instructions per pair);
+                                     0 (default) = fixed-dt path */
 };
 
 /* Bytes of DEVICE workspace needed for n_max particles and max_slabs sub-domains with the
@@ -156,6 +159,23 @@ int sph_interact(sph_ctx *ctx);
 
 /* a1-a8 in order; dt > 0. */
 int sph_step(sph_ctx *ctx, float dt);
+
+/* Variable time step (the step size "varies throughout each simulation according
+ * to the Courant-Friedrichs-Lewy (CFL) condition and the magnitude of the interactions", found
+ * with reductions over all particles; L222: every sub-domain determines its own dt_k and the
+ * minimum is used).  The paper prints no formula; reading A8b:
+ *     dt = cfl * min( sqrt(h / max_i |a_i|) over fluid particles,
+ *                     h / max_i (c_i + max_j |mu_ij|) over all particles ),  mu_ij as in L112.
+ * Needs the rates of an sph_interact made with SPH_OPT_ADAPTIVE_DT = 1 (else SPH_ERR_ORDER).
+ * HOST outputs, any may be NULL: *dt; amax_slab[n_slabs] = max |a| and smax_slab[n_slabs] =
+ * max (c + mu) of every current sub-domain (dt_k = cfl * min(sqrt(h/amax_k), h/smax_k)).
+ * One reduction kernel over the sorted arrays; synchronises the stream.  cfl > 0. */
+int sph_time_step(sph_ctx *ctx, float cfl, float *dt, float *amax_slab, float *smax_slab);
+
+/* a1-a7, sph_time_step, a8 with that step; *dt_used (HOST, may be NULL) receives it.  Turns
+ * SPH_OPT_ADAPTIVE_DT on.  Synchronises once per step (the step size crosses to the host, as
+ * the paper's does for its MPI_Allreduce). */
+int sph_step_adaptive(sph_ctx *ctx, float cfl, float *dt_used);
 
 int sph_get_view(sph_ctx *ctx, sph_view *out);
 

@@ -27,7 +27,10 @@
  *
  * Optional periodic box (minimum image) exists ONLY here, for the momentum pin.
  *
- * Pins: tests/test_oracle_physics.py (kernel integral, gradient vs finite difference,
+ *   time step    variable dt of reading A8b (orc_time_step below; L150, L222).
+ *
+ * Pins: tests/test_oracle_physics.py (time step: two-particle hand values, lattice expansion,
+ * per-slab minimum, numpy brute force; kernel integral, gradient vs finite difference,
  * EOS slope, divergence/pressure-gradient consistency, two-particle closed forms, pair
  * antisymmetry, brute force vs cell list, free fall, hydrostatic column).
  * Unpinned: absolute dam-break trajectories (the paper prints none) - "parity unpinned".

@@ -26,9 +26,10 @@ SPH_OK = 0
  SPH_T_VERLET, SPH_T_COUNT) = range(9)
 STAGE_NAMES = ["keys", "sort", "gather", "cells", "halo", "migrate", "interact", "verlet"]
 SPH_OPT_INTERACT_VARIANT = 0
+SPH_OPT_ADAPTIVE_DT = 1
 
 EXPORTS = ["sph_workspace_bytes", "sph_init", "sph_set_state", "sph_set_slabs", "sph_slab_planes_from_x",
-           "sph_sort_and_cells", "sph_build_halos", "sph_interact", "sph_step", "sph_get_view",
+           "sph_sort_and_cells", "sph_build_halos", "sph_interact", "sph_step", "sph_time_step", "sph_step_adaptive", "sph_get_view",
            "sph_download", "sph_status", "sph_set_option", "sph_profile_enable", "sph_profile_read",
            "sph_pair_stats", "sph_launch_count", "sph_destroy", "sph_strerror"]
 
@@ -74,6 +75,11 @@ _lib.sph_build_halos.restype = C.c_int
 _lib.sph_build_halos.argtypes = [C.c_void_p, C.POINTER(C.c_int32), C.c_int]
 _lib.sph_step.restype = C.c_int
 _lib.sph_step.argtypes = [C.c_void_p, C.c_float]
+_lib.sph_time_step.restype = C.c_int
+_lib.sph_time_step.argtypes = [C.c_void_p, C.c_float, C.POINTER(C.c_float), C.POINTER(C.c_float),
+                               C.POINTER(C.c_float)]
+_lib.sph_step_adaptive.restype = C.c_int
+_lib.sph_step_adaptive.argtypes = [C.c_void_p, C.c_float, C.POINTER(C.c_float)]
 _lib.sph_get_view.restype = C.c_int
 _lib.sph_get_view.argtypes = [C.c_void_p, C.POINTER(sph_view)]
 _lib.sph_download.restype = C.c_int
@@ -217,6 +223,20 @@ class Sph:
 
     def sph_step(self, dt: float):
         _check(_lib.sph_step(self._ctx, float(dt)))
+
+    def sph_time_step(self, cfl: float):
+        """(dt, amax_slab, smax_slab): variable time step and the per-sub-domain maxima it came from."""
+        dt = C.c_float(0.0)
+        am = (C.c_float * SPH_MAX_SLABS)()
+        sm = (C.c_float * SPH_MAX_SLABS)()
+        _check(_lib.sph_time_step(self._ctx, float(cfl), C.byref(dt), am, sm))
+        S = int(self.sph_get_view().n_slabs)
+        return float(dt.value), np.array(am[:S], dtype=np.float32), np.array(sm[:S], dtype=np.float32)
+
+    def sph_step_adaptive(self, cfl: float) -> float:
+        dt = C.c_float(0.0)
+        _check(_lib.sph_step_adaptive(self._ctx, float(cfl), C.byref(dt)))
+        return float(dt.value)
 
     def sph_status(self) -> int:
         return int(_lib.sph_status(self._ctx))

@@ -67,11 +67,13 @@ __device__ __forceinline__ float sound_speed(float rho, const PhysC &ph)
 
 // Adds the contribution of neighbour j to (ax, ay, az, dr); masses are applied by the caller
 // (mj = 1 in the uniform-mass path).  Branch-free: the viscous term uses min(v_ij.r_ij, 0).
-template <int KERNEL, bool GAMMA7>
+// MU: also track max_j |mu_ij| (variable time step, reading A8b) over the pairs with
+// r < 2h exactly (|mu| does not vanish at the edge of the support, unlike F) and mj != 0.
+template <int KERNEL, bool GAMMA7, bool MU>
 __device__ __forceinline__ void pair_term(float dx, float dy, float dz, float r2,
                                           float vxi, float vyi, float vzi, float rhoi, float Pi_, float ci,
                                           float4 vj, float Pj, float mj, const PhysC &ph,
-                                          float &ax, float &ay, float &az, float &dr)
+                                          float &ax, float &ay, float &az, float &dr, float &mumax)
 {
     float F = kernel_F<KERNEL>(r2, ph) * mj;
     float dvx = vxi - vj.x, dvy = vyi - vj.y, dvz = vzi - vj.z;
@@ -79,7 +81,13 @@ __device__ __forceinline__ void pair_term(float dx, float dy, float dz, float r2
     dr = fmaf(F, dot, dr);                                            // Eq. (7)
     // L112: Pi = -alpha cbar mu / rhobar = -alpha h (ci+cj) dot / ((r2+eta2)(rhoi+rhoj)) if dot < 0
     float cj = sound_speed<GAMMA7>(vj.w, ph);
-    float visc = -ph.alpha_h * (ci + cj) * fminf(dot, 0.0f) * rcp_fast((r2 + ph.eta2) * (rhoi + vj.w));
+    const float rsum = rhoi + vj.w;
+    const float rc = rcp_fast((r2 + ph.eta2) * rsum);
+    float visc = -ph.alpha_h * (ci + cj) * fminf(dot, 0.0f) * rc;
+    if (MU) {
+        const float mu = ph.h * fabsf(dot) * (rc * rsum);             // h |v_ij.r_ij| / (r2 + eta2)
+        mumax = fmaxf(mumax, (r2 < ph.four_h2 && mj != 0.0f) ? mu : 0.0f);
+    }
     float coef = -F * (Pi_ + Pj + visc);                              // Eq. (9)
     ax = fmaf(coef, dx, ax);
     ay = fmaf(coef, dy, ay);
@@ -87,14 +95,16 @@ __device__ __forceinline__ void pair_term(float dx, float dy, float dz, float r2
 }
 
 // ---- simple cross-check kernel -----------------------------------------------------------------
-template <int KERNEL, bool GAMMA7>
+template <int KERNEL, bool GAMMA7, bool MU>
 __global__ void __launch_bounds__(128)
 interact_simple_kernel(uint32_t n, const float4 *__restrict__ pos4, const float4 *__restrict__ velrho4,
                        const uint32_t *__restrict__ idt, const uint32_t *__restrict__ keyword,
-                       const uint32_t *__restrict__ cell_begin, float4 *__restrict__ acc4, GridC g, PhysC ph)
+                       const uint32_t *__restrict__ cell_begin, float4 *__restrict__ acc4, float *__restrict__ mu_out,
+                       GridC g, PhysC ph)
 {
     uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
+    float mumax = 0.f;
     float4 pi = pos4[i];
     float4 vi = velrho4[i];
     uint32_t cell = keyword[i] & CELL_MASK;
@@ -121,8 +131,8 @@ interact_simple_kernel(uint32_t n, const float4 *__restrict__ pos4, const float4
                     float4 vj = velrho4[j];
                     float mj = ph.uniform_mass ? ph.mass_fluid
                                                : ((idt[j] & TYPE_BIT) ? ph.mass_bound : ph.mass_fluid);
-                    pair_term<KERNEL, GAMMA7>(ddx, ddy, ddz, r2, vi.x, vi.y, vi.z, vi.w, pi.w, ci, vj, pj.w, mj, ph,
-                                      ax, ay, az, dr);
+                    pair_term<KERNEL, GAMMA7, MU>(ddx, ddy, ddz, r2, vi.x, vi.y, vi.z, vi.w, pi.w, ci, vj, pj.w, mj, ph,
+                                                  ax, ay, az, dr, mumax);
                 }
             }
         }
@@ -130,6 +140,7 @@ interact_simple_kernel(uint32_t n, const float4 *__restrict__ pos4, const float4
     if (fluid) { ax += ph.g[0]; ay += ph.g[1]; az += ph.g[2]; }
     else { ax = ay = az = 0.f; }
     acc4[i] = make_float4(ax, ay, az, dr);
+    if (MU) mu_out[i] = mumax;
 }
 
 // ---- staged production kernel --------------------------------------------------------------------
@@ -227,11 +238,11 @@ __device__ __forceinline__ float rel_origin(float corner, float reach)
     return __uint_as_float(__float_as_uint(corner) & ~3u);
 }
 
-template <int KERNEL, bool UNIFORM, bool GAMMA7>
+template <int KERNEL, bool UNIFORM, bool GAMMA7, bool MU>
 __global__ void __launch_bounds__(IA_THREADS, 2)
 interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict__ velrho4,
                        const uint32_t *__restrict__ idt, const uint32_t *__restrict__ keyword,
-                       const uint32_t *__restrict__ cell_begin, float4 *__restrict__ acc4,
+                       const uint32_t *__restrict__ cell_begin, float4 *__restrict__ acc4, float *__restrict__ mu_out,
                        GridC g, PhysC ph, int zb, int nzb, float thr_h /* filter threshold, units of h^2 */,
                        float zlim /* |z| bound the threshold was derived for, units of h */)
 {
@@ -312,7 +323,7 @@ interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict
         const __half2 hxi = __float2half2_rn(xs), hyi = __float2half2_rn(ys), hzi = __float2half2_rn(zs);
         const float ci = sound_speed<GAMMA7>(vi.w, ph);
         const int k_lo = max(kz - 1, 0), k_hi = min(kz + 2, nz);   // own 3-cell window in cbt rows
-        float ax = 0.f, ay = 0.f, az = 0.f, dr = 0.f;
+        float ax = 0.f, ay = 0.f, az = 0.f, dr = 0.f, mumax = 0.f;
         uint32_t sp = stk_base;                                     // shared address of the stack top
         uint32_t cur_mask = 0, cur_s = 0;                           // entry being drained
 
@@ -344,8 +355,8 @@ interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict
                 mj = ok ? (vj.w < 0.f ? ph.mass_bound : ph.mass_fluid) : 0.0f;
                 vj.w = fabsf(vj.w);
             }
-            pair_term<KERNEL, GAMMA7>(dx, dy, dz, r2, vi.x, vi.y, vi.z, vi.w, pi.w, ci, vj, rj.w, mj, ph,
-                                      ax, ay, az, dr);
+            pair_term<KERNEL, GAMMA7, MU>(dx, dy, dz, r2, vi.x, vi.y, vi.z, vi.w, pi.w, ci, vj, rj.w, mj, ph,
+                                          ax, ay, az, dr, mumax);
         };
         // one drain round: up to IA_DRAIN pending pairs per lane, as interleaved dependency chains
         auto drain_round = [&]() {
@@ -470,6 +481,7 @@ interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict
             if (fluid) { ax += ph.g[0]; ay += ph.g[1]; az += ph.g[2]; }
             else { ax = ay = az = 0.f; }
             acc4[i] = make_float4(ax, ay, az, dr);
+            if (MU) mu_out[i] = mumax;
         }
     }
 }
@@ -488,10 +500,10 @@ static void filter_threshold(int zb, float *thr_h, float *zlim)
     *zlim = (float)zl;
 }
 
-template <int KERNEL, bool UNIFORM, bool GAMMA7>
+template <int KERNEL, bool UNIFORM, bool GAMMA7, bool MU>
 static cudaError_t launch_staged(sph_ctx *c)
 {
-    auto kern = interact_staged_kernel<KERNEL, UNIFORM, GAMMA7>;
+    auto kern = interact_staged_kernel<KERNEL, UNIFORM, GAMMA7, MU>;
     static bool attr_set = false;
     if (!attr_set) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(IaSmem) + SPH_IA_PAD);
@@ -504,8 +516,8 @@ static cudaError_t launch_staged(sph_ctx *c)
     float thr_h, zlim;
     filter_threshold(zb, &thr_h, &zlim);
     kern<<<(uint32_t)blocks, IA_THREADS, sizeof(IaSmem) + SPH_IA_PAD, c->stream>>>(
-        c->pos4[c->cur], c->velrho4[c->cur], c->idt[c->cur], c->keyword, c->cell_begin, c->acc4, c->grid,
-        c->phys, zb, nzb, thr_h, zlim);
+        c->pos4[c->cur], c->velrho4[c->cur], c->idt[c->cur], c->keyword, c->cell_begin, c->acc4, c->mumax,
+        c->grid, c->phys, zb, nzb, thr_h, zlim);
     c->n_launches++;
     return cudaGetLastError();
 }
@@ -554,32 +566,39 @@ cudaError_t launch_pair_stats(sph_ctx *c, unsigned long long *d_out)
     return cudaGetLastError();
 }
 
-template <int KERNEL, bool GAMMA7>
+template <int KERNEL, bool GAMMA7, bool MU>
 static cudaError_t launch_simple(sph_ctx *c)
 {
     uint32_t n = (uint32_t)c->n;
-    interact_simple_kernel<KERNEL, GAMMA7><<<(n + 127) / 128, 128, 0, c->stream>>>(
-        n, c->pos4[c->cur], c->velrho4[c->cur], c->idt[c->cur], c->keyword, c->cell_begin, c->acc4, c->grid,
-        c->phys);
+    interact_simple_kernel<KERNEL, GAMMA7, MU><<<(n + 127) / 128, 128, 0, c->stream>>>(
+        n, c->pos4[c->cur], c->velrho4[c->cur], c->idt[c->cur], c->keyword, c->cell_begin, c->acc4, c->mumax,
+        c->grid, c->phys);
     c->n_launches++;
     return cudaGetLastError();
 }
 
-cudaError_t launch_interact(sph_ctx *c)
+template <bool MU>
+static cudaError_t launch_interact_mu(sph_ctx *c)
 {
-    if (c->n == 0) return cudaSuccess;
     const bool uni = c->phys.uniform_mass != 0, g7 = c->phys.gamma == 7;
     const int k = c->phys.kernel;
     if (c->interact_variant == 1) {
-        if (k == 0) return g7 ? launch_simple<0, true>(c) : launch_simple<0, false>(c);
-        return g7 ? launch_simple<1, true>(c) : launch_simple<1, false>(c);
+        if (k == 0) return g7 ? launch_simple<0, true, MU>(c) : launch_simple<0, false, MU>(c);
+        return g7 ? launch_simple<1, true, MU>(c) : launch_simple<1, false, MU>(c);
     }
     if (k == 0) {
-        if (uni) return g7 ? launch_staged<0, true, true>(c) : launch_staged<0, true, false>(c);
-        return g7 ? launch_staged<0, false, true>(c) : launch_staged<0, false, false>(c);
+        if (uni) return g7 ? launch_staged<0, true, true, MU>(c) : launch_staged<0, true, false, MU>(c);
+        return g7 ? launch_staged<0, false, true, MU>(c) : launch_staged<0, false, false, MU>(c);
     }
-    if (uni) return g7 ? launch_staged<1, true, true>(c) : launch_staged<1, true, false>(c);
-    return g7 ? launch_staged<1, false, true>(c) : launch_staged<1, false, false>(c);
+    if (uni) return g7 ? launch_staged<1, true, true, MU>(c) : launch_staged<1, true, false, MU>(c);
+    return g7 ? launch_staged<1, false, true, MU>(c) : launch_staged<1, false, false, MU>(c);
+}
+
+// with_mu: also write max_j |mu_ij| per particle (needed by the variable time step only)
+cudaError_t launch_interact(sph_ctx *c, bool with_mu)
+{
+    if (c->n == 0) return cudaSuccess;
+    return with_mu ? launch_interact_mu<true>(c) : launch_interact_mu<false>(c);
 }
 
 }  // namespace sph

@@ -15,7 +15,7 @@ constexpr size_t ALIGN = 256;
 size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 
 struct Layout {
-    size_t pos4[2], velrho4[2], velrhoM1[2], idt[2], acc4, kv[2], keyword, hist, tile_state, counters,
+    size_t pos4[2], velrho4[2], velrhoM1[2], idt[2], acc4, mumax, dt_red, kv[2], keyword, hist, tile_state, counters,
         cell_begin, gap_list, mig_tile, mig_grp, mig_off, scratch64, slab_begin, halo_range, halo_offset, halo_pos4, halo_velrho4, halo_idt,
         migrants, mig_total, mig_count, prev_init, flags, total;
 };
@@ -54,6 +54,8 @@ bool make_layout(const sph_params *p, uint64_t n, int max_slabs, Layout *L)
         L->idt[b] = take(4 * nn);
     }
     L->acc4 = take(16 * nn);
+    L->mumax = take(4 * nn);
+    L->dt_red = take(4 * 2 * SPH_MAX_SLABS);
     L->kv[0] = take(8 * nn);
     L->kv[1] = take(8 * nn);
     L->keyword = take(4 * nn);
@@ -199,7 +201,7 @@ int upload_state(sph_ctx *c, const sph_particles *part)
     CK(c, launch_init_state(c, dpos, dvel, drho, dtype));
     if (!part->on_device) CK(c, cudaStreamSynchronize(c->stream));   // host arrays may be reused
     c->have_prev_ranges = false;
-    c->sorted_valid = c->halos_valid = c->rates_valid = false;
+    c->sorted_valid = c->halos_valid = c->rates_valid = c->mu_valid = false;
     c->step_index = 0;
     return SPH_OK;
 }
@@ -265,6 +267,10 @@ int sph_init(sph_ctx **out, const sph_params *p, const sph_particles *part, int 
         c->kv[b] = (uint2 *)(w + L.kv[b]);
     }
     c->acc4 = (float4 *)(w + L.acc4);
+    c->mumax = (float *)(w + L.mumax);
+    c->dt_red = (uint32_t *)(w + L.dt_red);
+    c->adaptive_dt = 0;
+    c->mu_valid = false;
     c->keyword = (uint32_t *)(w + L.keyword);
     c->hist = (uint32_t *)(w + L.hist);
     c->tile_state = (uint32_t *)(w + L.tile_state);
@@ -367,6 +373,7 @@ int sph_sort_and_cells(sph_ctx *c)
     c->sorted_valid = true;
     c->halos_valid = false;
     c->rates_valid = false;
+    c->mu_valid = false;
     return SPH_OK;
 }
 
@@ -402,8 +409,25 @@ int sph_interact(sph_ctx *c)
     if (c->sticky) return c->sticky;
     if (!c->sorted_valid) return SPH_ERR_ORDER;
     Timed t(c, SPH_T_INTERACT);
-    CK(c, launch_interact(c));
+    CK(c, launch_interact(c, c->adaptive_dt != 0));
     c->rates_valid = true;
+    c->mu_valid = c->adaptive_dt != 0;
+    return SPH_OK;
+}
+
+static int verlet_and_advance(sph_ctx *c, float dt)
+{
+    {
+        Timed t(c, SPH_T_VERLET);
+        int ns = c->P.verlet_ns;
+        int corrective = ns <= 0 ? (c->step_index == 0) : (c->step_index % (uint64_t)ns == 0);
+        CK(c, launch_verlet(c, dt, corrective));
+    }
+    c->step_index++;
+    c->sorted_valid = false;      // positions moved: the cell table no longer matches them
+    c->halos_valid = false;
+    c->rates_valid = false;
+    c->mu_valid = false;
     return SPH_OK;
 }
 
@@ -417,16 +441,58 @@ int sph_step(sph_ctx *c, float dt)
     if (rc != SPH_OK) return rc;
     rc = sph_interact(c);
     if (rc != SPH_OK) return rc;
+    return verlet_and_advance(c, dt);
+}
+
+int sph_time_step(sph_ctx *c, float cfl, float *dt, float *amax_slab, float *smax_slab)
+{
+    if (!c || !(cfl > 0.f) || !isfinite(cfl)) return SPH_ERR_ARG;
+    if (c->sticky) return c->sticky;
+    if (!c->sorted_valid || !c->rates_valid || !c->mu_valid) return SPH_ERR_ORDER;
+    uint32_t h[2 * SPH_MAX_SLABS];
     {
         Timed t(c, SPH_T_VERLET);
-        int ns = c->P.verlet_ns;
-        int corrective = ns <= 0 ? (c->step_index == 0) : (c->step_index % (uint64_t)ns == 0);
-        CK(c, launch_verlet(c, dt, corrective));
+        CK(c, launch_dt_reduce(c));
     }
-    c->step_index++;
-    c->sorted_valid = false;      // positions moved: the cell table no longer matches them
-    c->halos_valid = false;
+    CK(c, cudaMemcpyAsync(h, c->dt_red, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    CK(c, cudaStreamSynchronize(c->stream));
+    const int S = c->tagged_slabs.n_slabs;
+    float amax = 0.f, smax = 0.f;
+    for (int k = 0; k < S; ++k) {
+        float a2, sg;
+        memcpy(&a2, &h[2 * k], 4);
+        memcpy(&sg, &h[2 * k + 1], 4);
+        const float a = sqrtf(a2);
+        if (amax_slab) amax_slab[k] = a;
+        if (smax_slab) smax_slab[k] = sg;
+        if (a > amax) amax = a;
+        if (sg > smax) smax = sg;
+    }
+    if (dt) {
+        const double hh = (double)c->P.h;
+        const double dt_f = amax > 0.f ? sqrt(hh / (double)amax) : INFINITY;
+        const double dt_cv = smax > 0.f ? hh / (double)smax : INFINITY;
+        *dt = (float)((double)cfl * (dt_f < dt_cv ? dt_f : dt_cv));
+    }
     return SPH_OK;
+}
+
+int sph_step_adaptive(sph_ctx *c, float cfl, float *dt_used)
+{
+    if (!c || !(cfl > 0.f) || !isfinite(cfl)) return SPH_ERR_ARG;
+    c->adaptive_dt = 1;
+    int rc = sph_sort_and_cells(c);
+    if (rc != SPH_OK) return rc;
+    rc = sph_build_halos(c, nullptr, 0);
+    if (rc != SPH_OK) return rc;
+    rc = sph_interact(c);
+    if (rc != SPH_OK) return rc;
+    float dt = 0.f;
+    rc = sph_time_step(c, cfl, &dt, nullptr, nullptr);
+    if (rc != SPH_OK) return rc;
+    if (!(dt > 0.f) || !isfinite(dt)) return SPH_ERR_NONFINITE;
+    if (dt_used) *dt_used = dt;
+    return verlet_and_advance(c, dt);
 }
 
 int sph_get_view(sph_ctx *c, sph_view *v)
@@ -497,6 +563,10 @@ int sph_set_option(sph_ctx *c, int option, int value)
     case SPH_OPT_INTERACT_VARIANT:
         if (value != 0 && value != 1) return SPH_ERR_ARG;
         c->interact_variant = value;
+        return SPH_OK;
+    case SPH_OPT_ADAPTIVE_DT:
+        if (value != 0 && value != 1) return SPH_ERR_ARG;
+        c->adaptive_dt = value;
         return SPH_OK;
     default:
         return SPH_ERR_ARG;

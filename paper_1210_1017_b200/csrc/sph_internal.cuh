@@ -76,6 +76,8 @@ struct sph_ctx {
     uint32_t *idt[2];
     int cur;
     float4 *acc4;
+    float *mumax;              // max_j |mu_ij| per particle (sorted order), written when adaptive_dt is set
+    uint32_t *dt_red;          // 2 * SPH_MAX_SLABS float bit patterns: per slab max |a|^2 (fluid), max (c + mu)
     // sort
     uint2 *kv[2];              // (keyword, prevSlab<<28 | sourceIndex)
     int kv_sorted;             // which kv buffer holds the sorted pairs
@@ -106,6 +108,8 @@ struct sph_ctx {
     bool sorted_valid;         // arrays sorted + cell table valid for the current positions
     bool halos_valid;
     bool rates_valid;
+    bool mu_valid;             // mumax belongs to the current rates
+    int adaptive_dt;           // SPH_OPT_ADAPTIVE_DT: sph_interact also produces mumax
     uint64_t step_index;
     int interact_variant;
     int zblock;                // cells per z-block of the staged interaction kernel
@@ -128,7 +132,8 @@ cudaError_t launch_slab_meta(sph_ctx *c);
 cudaError_t launch_retag(sph_ctx *c);
 cudaError_t launch_halo_gather(sph_ctx *c);
 cudaError_t launch_migrants(sph_ctx *c);
-cudaError_t launch_interact(sph_ctx *c);
+cudaError_t launch_interact(sph_ctx *c, bool with_mu);
+cudaError_t launch_dt_reduce(sph_ctx *c);
 cudaError_t launch_verlet(sph_ctx *c, float dt, int corrective);
 cudaError_t launch_pair_stats(sph_ctx *c, unsigned long long *d_out);
 cudaError_t launch_download_pack(sph_ctx *c, float *pos3, float *vel3, float *rho, float *acc3,

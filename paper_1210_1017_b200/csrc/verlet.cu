@@ -83,4 +83,73 @@ cudaError_t launch_download_pack(sph_ctx *c, float *pos3, float *vel3, float *rh
     return cudaGetLastError();
 }
 
+// ---- variable time step: per-sub-domain maxima ("minimum and maximum values of certain
+// physical quantities need to be found among all particles, and for this, efficient CUDA reduction
+// algorithms ... are employed"; L222: every sub-domain finds its own dt_k, the step uses the minimum).
+// Reading A8b: dt = cfl * min( sqrt(h / max|a|) over fluid, h / max(c_i + max_j |mu_ij|) over all ).
+// Slabs are contiguous ranges of the sorted order, so a thread finds its slab in the range table; the
+// maxima of non-negative floats are taken on their bit patterns (shared, then global atomicMax).
+// HBM-bound: reads acc4 (16 B), rho (velrho4, 16 B), mumax (4 B), idt (4 B) per particle.
+__global__ void __launch_bounds__(256)
+dt_reduce_kernel(uint32_t n, const float4 *__restrict__ acc4, const float4 *__restrict__ velrho4,
+                 const float *__restrict__ mumax, const uint32_t *__restrict__ idt,
+                 const uint32_t *__restrict__ slab_begin, int n_slabs, PhysC ph, uint32_t *__restrict__ red)
+{
+    __shared__ uint32_t s_begin[SPH_MAX_SLABS + 1];
+    __shared__ uint32_t s_red[2 * SPH_MAX_SLABS];
+    if (threadIdx.x <= SPH_MAX_SLABS) s_begin[threadIdx.x] = threadIdx.x <= (uint32_t)n_slabs ? slab_begin[threadIdx.x] : 0xFFFFFFFFu;
+    if (threadIdx.x < 2 * SPH_MAX_SLABS) s_red[threadIdx.x] = 0u;
+    __syncthreads();
+    // the loop bound is warp-uniform (whole warps iterate together; lanes past n are masked), because
+    // the body uses full-mask warp collectives
+    for (uint32_t i0 = blockIdx.x * blockDim.x + (threadIdx.x & ~31u); i0 < n; i0 += gridDim.x * blockDim.x) {
+        const uint32_t i = i0 + (threadIdx.x & 31u);
+        const bool valid = i < n;
+        float sig = 0.0f, a2 = 0.0f;
+        int s = 0;
+        if (valid) {
+            const float4 a = __ldg(acc4 + i);
+            const float rho = __ldg(velrho4 + i).w;
+            const bool fluid = (__ldg(idt + i) & TYPE_BIT) == 0;
+            const float x = rho * ph.inv_rho0;
+            const float c = ph.gamma == 7 ? ph.c0 * x * x * x : ph.c0 * __powf(x, 0.5f * (float)(ph.gamma - 1));
+            sig = c + __ldg(mumax + i);
+            a2 = fluid ? fmaf(a.z, a.z, fmaf(a.y, a.y, a.x * a.x)) : 0.0f;
+            for (int k = 1; k < n_slabs; ++k) s += (i >= s_begin[k]) ? 1 : 0;
+        }
+        // warp-level pre-reduction when the whole warp sits in one slab (almost always)
+        const int s0 = __shfl_sync(0xffffffffu, s, 0);
+        if (__all_sync(0xffffffffu, !valid || s == s0)) {
+            float ma = a2, ms = sig;
+#pragma unroll
+            for (int o = 16; o; o >>= 1) {
+                ma = fmaxf(ma, __shfl_xor_sync(0xffffffffu, ma, o));
+                ms = fmaxf(ms, __shfl_xor_sync(0xffffffffu, ms, o));
+            }
+            if ((threadIdx.x & 31) == 0) {
+                atomicMax(&s_red[2 * s0], __float_as_uint(ma));
+                atomicMax(&s_red[2 * s0 + 1], __float_as_uint(ms));
+            }
+        } else if (valid) {
+            atomicMax(&s_red[2 * s], __float_as_uint(a2));
+            atomicMax(&s_red[2 * s + 1], __float_as_uint(sig));
+        }
+    }
+    __syncthreads();
+    if (threadIdx.x < 2 * SPH_MAX_SLABS && s_red[threadIdx.x]) atomicMax(&red[threadIdx.x], s_red[threadIdx.x]);
+}
+
+cudaError_t launch_dt_reduce(sph_ctx *c)
+{
+    uint32_t n = (uint32_t)c->n;
+    cudaError_t e = cudaMemsetAsync(c->dt_red, 0, sizeof(uint32_t) * 2 * SPH_MAX_SLABS, c->stream);
+    if (e != cudaSuccess || n == 0) return e;
+    uint32_t blocks = (n + 255) / 256;
+    if (blocks > (uint32_t)NUM_SMS * 8) blocks = NUM_SMS * 8;
+    dt_reduce_kernel<<<blocks, 256, 0, c->stream>>>(n, c->acc4, c->velrho4[c->cur], c->mumax, c->idt[c->cur],
+                                                   c->slab_begin, c->tagged_slabs.n_slabs, c->phys, c->dt_red);
+    c->n_launches++;
+    return cudaGetLastError();
+}
+
 }  // namespace sph
