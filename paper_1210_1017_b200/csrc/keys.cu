@@ -68,6 +68,7 @@ __device__ __forceinline__ int upper_slot(const T *table, T x)
 
 // prev_mode: 0 = none (no migrants), 1 = previous slab ranges over the current order,
 //            2 = caller-supplied prev_init[id]
+constexpr int KEYS_CX_TAB = 4096;    // cell planes along x covered by the shared-memory slab table
 constexpr int KEYS_IPT = 4;          // particles per thread per iteration (independent loads in flight)
 
 template <int PASSES>
@@ -78,8 +79,9 @@ keys_kernel(uint32_t n, const float4 *__restrict__ pos4, const uint32_t *__restr
             const uint8_t *__restrict__ prev_init)
 {
     __shared__ uint32_t s_hist[PASSES * 256];
-    __shared__ uint32_t s_prev_begin[SPH_MAX_SLABS + 1];
+    __shared__ uint32_t s_prev_begin[SPH_MAX_SLABS + 2];
     __shared__ int s_planes[SPH_MAX_SLABS + 2];
+    __shared__ uint8_t s_cx_tab[KEYS_CX_TAB];     // slab | edge label << 4 of every cell plane (if nc[0] fits)
     for (int k = threadIdx.x; k < PASSES * 256; k += blockDim.x) s_hist[k] = 0;
     if (threadIdx.x <= SPH_MAX_SLABS) {
         const int t = threadIdx.x;
@@ -88,14 +90,27 @@ keys_kernel(uint32_t n, const float4 *__restrict__ pos4, const uint32_t *__restr
         if (t == 0) { s_planes[SPH_MAX_SLABS + 1] = 0x7fffffff; s_prev_begin[0] = 0; }
     }
     __syncthreads();
+    const int S = sl.n_slabs;
+    const bool use_tab = g.nc[0] <= KEYS_CX_TAB;
+    if (use_tab) {
+        for (int cx = threadIdx.x; cx < g.nc[0]; cx += blockDim.x) {
+            const int slab = upper_slot(s_planes, cx);
+            uint32_t lab = 0;                                          // edge label (L240)
+            if (slab > 0 && cx == s_planes[slab]) lab = 1;
+            if (slab < S - 1 && cx == s_planes[slab + 1] - 1) lab = 2;
+            s_cx_tab[cx] = (uint8_t)(slab | (lab << 4));
+        }
+        __syncthreads();
+    }
 
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const uint32_t lt_mask = (1u << lane) - 1u;
-    const int S = sl.n_slabs;
     constexpr uint32_t WCHUNK = 32 * KEYS_IPT;
     const uint32_t stride = gridDim.x * (blockDim.x >> 5) * WCHUNK;
     // a warp owns WCHUNK consecutive particles per iteration; the loop bound is warp-uniform, so
     // the warp stays converged for match_any
+    int prev_s = 0;
+    uint32_t prev_lo = 1, prev_hi = 0;            // empty range: the first particle searches
     for (uint32_t base = (blockIdx.x * (blockDim.x >> 5) + warp) * WCHUNK; base < n; base += stride) {
         float4 p[KEYS_IPT];
         uint32_t w[KEYS_IPT];
@@ -117,13 +132,28 @@ keys_kernel(uint32_t n, const float4 *__restrict__ pos4, const uint32_t *__restr
                 const int cy = cell_coord(p[k].y, g.min[1], g.inv_cell, g.nc[1]);
                 const int cz = cell_coord(p[k].z, g.min[2], g.inv_cell, g.nc[2]);
                 cell = (uint32_t)((cx * g.nc[1] + cy) * g.nc[2] + cz);
-                const int slab = upper_slot(s_planes, cx);
+                int slab;
                 uint32_t lab = 0;                                          // edge label (L240)
-                if (slab > 0 && cx == s_planes[slab]) lab = 1;
-                if (slab < S - 1 && cx == s_planes[slab + 1] - 1) lab = 2;
+                if (use_tab) {
+                    const uint32_t t = s_cx_tab[cx];
+                    slab = (int)(t & 15u);
+                    lab = t >> 4;
+                } else {
+                    slab = upper_slot(s_planes, cx);
+                    if (slab > 0 && cx == s_planes[slab]) lab = 1;
+                    if (slab < S - 1 && cx == s_planes[slab + 1] - 1) lab = 2;
+                }
                 int prev = slab;
-                if (prev_mode == 1) prev = upper_slot(s_prev_begin, i);
-                else if (prev_mode == 2) prev = min((int)prev_init[id], S - 1);
+                if (prev_mode == 1) {
+                    // previous owner = slab range of the current index; consecutive indices almost
+                    // always stay in the range found last
+                    if (i < prev_lo || i >= prev_hi) {
+                        prev_s = upper_slot(s_prev_begin, i);
+                        prev_lo = s_prev_begin[prev_s];
+                        prev_hi = s_prev_begin[prev_s + 1];
+                    }
+                    prev = prev_s;
+                } else if (prev_mode == 2) prev = min((int)prev_init[id], S - 1);
                 const uint32_t mig = slab < prev ? 1u : (slab > prev ? 2u : 0u);   // migration label (L264)
                 const uint32_t tag = lab | (mig << 2);
                 kv_by_id[id] = make_uint2((tag << TAG_SHIFT) | cell, ((uint32_t)prev << 28) | i);
@@ -134,8 +164,15 @@ keys_kernel(uint32_t n, const float4 *__restrict__ pos4, const uint32_t *__restr
             // Otherwise (random keys): one plain shared-memory atomic per key - with ~28 distinct
             // digits among 32 lanes they hardly collide, measured 2.4 cycles per warp instruction.
             const uint32_t vmask = __ballot_sync(0xffffffffu, valid);
+            // valid lanes are a prefix of the warp, so lane 0 speaks for a warp that has any
+            const uint32_t c0 = __shfl_sync(0xffffffffu, cell, 0);
+            const bool upper_uniform = __all_sync(0xffffffffu, !valid || (cell >> 8) == (c0 >> 8));
 #pragma unroll
             for (int q = 0; q < PASSES; ++q) {
+                if (q > 0 && upper_uniform) {             // one test covers all the upper digits
+                    if (lane == 0 && vmask) atomicAdd(&s_hist[q * 256 + ((c0 >> (8 * q)) & 255u)], __popc(vmask));
+                    continue;
+                }
                 const uint32_t d = valid ? ((cell >> (8 * q)) & 255u) : 256u;
                 const uint32_t prev = __shfl_up_sync(0xffffffffu, d, 1);
                 const uint32_t runs = __ballot_sync(0xffffffffu, d != prev);   // lane 0: compares with itself
