@@ -25,10 +25,10 @@ def test_config0_sort_cells_single_slab():
     assert len(A["migrants"]) == 0
 
 
-@pytest.mark.parametrize("n", [1 << 16, 100003, 6144, 6145, 1, 37])
+@pytest.mark.parametrize("n", [1 << 16, 100003, 8191, 8192, 8193, 4095, 4097, 255, 256, 257, 1, 37])
 def test_uniform_cube_sort_halos_migrants(n):
     """Random keys, 8 slabs, synthetic previous owners: several radix tiles and ragged tails
-    (6144 = one tile exactly, 6145 = one tile + 1)."""
+    (8192 = one radix tile exactly, 4096 = one migrant group, 256 = one gather tile, each also +-1)."""
     w = W.uniform_cube(n)
     nc = OA.grid_dims(w.params["dom_min"], w.params["dom_max"], w.params["h"])
     S = 8 if nc[0] >= 16 else 1
