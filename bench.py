@@ -186,14 +186,21 @@ def run_micro(args):
     passes = (v.cell_bits + 7) // 8
     med = {k: float(np.median(x)) for k, x in acc.items() if np.sum(x) > 0}
     byts = dict(keys=BYTES["keys"] * n, sort=BYTES["sort_per_pass"] * passes * n, gather=BYTES["gather"] * n,
-                cells=8.0 * (v.ncells + 1), halo=72.0 * n_halo, migrate=4.0 * n + 16.0 * n_mig)
+                cells=None, halo=72.0 * n_halo, migrate=4.0 * n + 16.0 * n_mig)
     out = dict(workload=w.name, n=n, cell_bits=v.cell_bits, passes=passes, n_halo=n_halo, n_migrants=n_mig,
                sort_gkeys_s=n / (med["sort"] * 1e-3) / 1e9,
                sort_with_keys_gkeys_s=n / ((med["sort"] + med["keys"]) * 1e-3) / 1e9,
                hbm_peak_gbs=pk["hbm_gbs"], peak_source=pk["source"],
-               stages={k: dict(ms=med[k], algorithmic_gbs=byts[k] / (med[k] * 1e-3) / 1e9,
-                               frac_of_hbm_peak=byts[k] / (med[k] * 1e-3) / 1e9 / pk["hbm_gbs"])
+               stages={k: (dict(ms=med[k], algorithmic_gbs=byts[k] / (med[k] * 1e-3) / 1e9,
+                                frac_of_hbm_peak=byts[k] / (med[k] * 1e-3) / 1e9 / pk["hbm_gbs"])
+                           if byts[k] is not None else dict(ms=med[k]))
                        for k in med if k in byts})
+    # the cell table is written by the gather kernel (short gaps) and the gap-fill kernel of the
+    # "cells" stage (long runs of empty cells): one combined figure, 4 B written per cell
+    gc_ms = med["gather"] + med["cells"]
+    gc_b = byts["gather"] + 4.0 * (v.ncells + 1)
+    out["stages"]["gather+cells"] = dict(ms=gc_ms, algorithmic_gbs=gc_b / (gc_ms * 1e-3) / 1e9,
+                                         frac_of_hbm_peak=gc_b / (gc_ms * 1e-3) / 1e9 / pk["hbm_gbs"])
     print(json.dumps(out))
 
 
@@ -367,7 +374,7 @@ def main():
     n_halo = int(T["halo_offset"][-1].item()) if w.n_slabs > 1 else 0
     n_mig = int(T["mig_total"].item())
     byts = dict(keys=BYTES["keys"] * n, sort=BYTES["sort_per_pass"] * passes * n, gather=BYTES["gather"] * n,
-                cells=8.0 * (v.ncells + 1), halo=72.0 * n_halo, migrate=4.0 * n + 16.0 * n_mig,
+                cells=None, halo=72.0 * n_halo, migrate=4.0 * n + 16.0 * n_mig,
                 verlet=BYTES["verlet"] * n)
     stages = {}
     for k, (ms, c) in stage.items():
@@ -375,11 +382,16 @@ def main():
             continue
         avg = ms / c
         d = dict(ms=avg, share=ms / ms_total)
-        if k in byts:
+        if byts.get(k) is not None:
             gbs = byts[k] / (avg * 1e-3) / 1e9
             d.update(algorithmic_gbs=gbs, frac_of_hbm_peak=gbs / pk["hbm_gbs"])
         stages[k] = d
-
+    if "gather" in stages and "cells" in stages:      # see run_micro: one combined figure for a3 + a4
+        gc_ms = stages["gather"]["ms"] + stages["cells"]["ms"]
+        gc_b = byts["gather"] + 4.0 * (v.ncells + 1)
+        stages["gather+cells"] = dict(ms=gc_ms, share=gc_ms * args.steps / ms_total,
+                                      algorithmic_gbs=gc_b / (gc_ms * 1e-3) / 1e9,
+                                      frac_of_hbm_peak=gc_b / (gc_ms * 1e-3) / 1e9 / pk["hbm_gbs"])
     cpu = None
     if not args.no_cpu_baseline:
         oracle_step_sample(w, 20_000)                         # builds / warms the oracle library

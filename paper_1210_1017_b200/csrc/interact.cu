@@ -186,7 +186,6 @@ struct IaSmem {
     int32_t stage_off[9];                     // smem index = global index + stage_off
 };
 
-size_t interact_smem_bytes(const sph_ctx *) { return sizeof(IaSmem); }
 int interact_threads() { return IA_THREADS; }
 
 __device__ __forceinline__ void sts_u32(uint32_t addr, uint32_t v)

@@ -143,7 +143,6 @@ uint32_t radix_tiles(uint64_t n);
 uint32_t gather_tiles(uint64_t n);
 uint32_t mig_groups(uint64_t n);
 size_t gap_list_entries(uint64_t ncells);
-size_t interact_smem_bytes(const sph_ctx *c);
 int interact_threads();
 
 // Tait pressure over rho^2 from rho, fp32, cancellation-free.
@@ -156,73 +155,8 @@ __device__ __forceinline__ float tait_p_over_rho2(float rho, const PhysC &ph)
     return __fdividef(p, rho * rho);
 }
 
-// ---- warp match on an 8-bit digit -----------------------------------------------------------
-// Mask of the lanes whose digit equals this lane's (lanes with valid == false match nobody and
-// are matched by nobody).  The hardware MATCH.ANY serialises over the distinct values in the
-// warp: fast for the long runs of equal digits of a running simulation (particles arrive almost
-// sorted), slow for random digits (measured: the ranking loop of the radix sort spent > 40 % of
-// the kernel waiting on it).  So: count the run boundaries between neighbouring lanes (one
-// shuffle + one ballot); few runs -> MATCH.ANY, many -> eight ballots, whose cost does not
-// depend on the distribution and pipelines across the items of a thread.  Warp-uniform branch.
+// Warps with at most this many runs of equal digits use the hardware MATCH.ANY (about 8 cycles per
+// distinct value) for their histogram contribution; beyond it plain shared-memory atomics win.
 constexpr int MATCH_MAX_RUNS = 6;
-
-__device__ __forceinline__ uint32_t warp_match8(uint32_t digit, bool valid)
-{
-    const uint32_t key = valid ? digit : 256u;                       // all invalid lanes form one run
-    const uint32_t prev = __shfl_up_sync(0xffffffffu, key, 1);
-    const uint32_t runs = __ballot_sync(0xffffffffu, key != prev);   // lane 0 compares with itself: 0
-    const uint32_t vmask = __ballot_sync(0xffffffffu, valid);
-    if (__popc(runs) <= MATCH_MAX_RUNS) return __match_any_sync(0xffffffffu, key) & vmask;
-    uint32_t m = vmask;
-#pragma unroll
-    for (int b = 0; b < 8; ++b) {
-        const bool bit = (digit >> b) & 1u;
-        const uint32_t bal = __ballot_sync(0xffffffffu, bit);
-        m &= bit ? bal : ~bal;
-    }
-    return m;
-}
-
-// ---- decoupled look-back of a chained scan, one warp per tile ---------------------------------
-// state[t] = flag << 32 | value, flag 0 = not published, 1 = tile aggregate, 2 = inclusive prefix.
-__device__ __forceinline__ unsigned long long ld_relaxed_u64(const unsigned long long *p)
-{
-    unsigned long long v;
-    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
-    return v;
-}
-__device__ __forceinline__ void st_relaxed_u64(unsigned long long *p, unsigned long long v)
-{
-    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
-}
-
-// Called by all 32 lanes of ONE warp: combines (with op) the values of the tiles before `tile`
-// back to the nearest inclusive prefix, 32 predecessors per round trip.  Returns the exclusive
-// carry of `tile` in every lane.
-template <typename Op>
-__device__ __forceinline__ uint32_t warp_lookback(const unsigned long long *state, uint32_t tile, uint32_t identity,
-                                                  Op op)
-{
-    const uint32_t lane = threadIdx.x & 31;
-    uint32_t carry = identity;
-    int t = (int)tile - 1;
-    while (t >= 0) {
-        const int tt = t - (int)lane;
-        const unsigned long long s = tt >= 0 ? ld_relaxed_u64(state + tt) : ((2ull << 32) | identity);
-        const uint32_t flag = (uint32_t)(s >> 32);
-        const uint32_t not_ready = __ballot_sync(0xffffffffu, flag == 0);
-        const uint32_t inc = __ballot_sync(0xffffffffu, flag == 2);
-        const int first_inc = inc ? (__ffs(inc) - 1) : 31;
-        const uint32_t need = first_inc >= 31 ? 0xffffffffu : ((2u << first_inc) - 1u);
-        if (not_ready & need) continue;                        // poll the same window again
-        uint32_t v = ((int)lane <= first_inc) ? (uint32_t)s : identity;
-#pragma unroll
-        for (int o = 16; o; o >>= 1) v = op(v, __shfl_xor_sync(0xffffffffu, v, o));
-        carry = op(carry, v);
-        if (inc) break;
-        t -= 32;
-    }
-    return carry;
-}
 
 }  // namespace sph
