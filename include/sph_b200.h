@@ -120,7 +120,8 @@ enum {
 /* Options for sph_set_option. */
 enum {
     SPH_OPT_INTERACT_VARIANT = 0, /* 0 = smem-staged production kernel, 1 = simple
-                                     one-thread-per-particle kernel (cross-check) */
+                                     one-thread-per-particle kernel (cross-check), 2 = staged
+                                     kernel over tiles of 2 x 2 columns (cross-check) */
     SPH_OPT_ADAPTIVE_DT = 1       /* 1 = sph_interact also records max_j |mu_ij| of every particle,
                                      which sph_time_step needs (costs a few instructions per pair);
                                      0 (default) = fixed-dt path */

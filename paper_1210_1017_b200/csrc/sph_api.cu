@@ -300,6 +300,10 @@ int sph_init(sph_ctx **out, const sph_params *p, const sph_particles *part, int 
     if (zb < 1) zb = 1;
     if (zb > 32) zb = 32;
     c->zblock = zb;
+    int zt = (int)floor((double)interact_tile_threads() * 0.97 / ((ppc > 0.05 ? ppc : 0.05) * interact_tile_columns()));
+    if (zt < 1) zt = 1;
+    if (zt > interact_tile_zmax()) zt = interact_tile_zmax();
+    c->zblock_tile = zt;
 
     cudaError_t e = cudaMemsetAsync(c->acc4, 0, 16 * (c->n ? c->n : 1), c->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->mig_total, 0, 4, c->stream);
@@ -561,7 +565,7 @@ int sph_set_option(sph_ctx *c, int option, int value)
     if (!c) return SPH_ERR_ARG;
     switch (option) {
     case SPH_OPT_INTERACT_VARIANT:
-        if (value != 0 && value != 1) return SPH_ERR_ARG;
+        if (value < 0 || value > 2) return SPH_ERR_ARG;
         c->interact_variant = value;
         return SPH_OK;
     case SPH_OPT_ADAPTIVE_DT:

@@ -113,6 +113,7 @@ struct sph_ctx {
     uint64_t step_index;
     int interact_variant;
     int zblock;                // cells per z-block of the staged interaction kernel
+    int zblock_tile;           // same for the tile variant
 
     uint64_t n_launches;       // kernels launched so far (memsets and copies not counted)
 
@@ -144,6 +145,9 @@ uint32_t gather_tiles(uint64_t n);
 uint32_t mig_groups(uint64_t n);
 size_t gap_list_entries(uint64_t ncells);
 int interact_threads();
+int interact_tile_threads();
+int interact_tile_columns();
+int interact_tile_zmax();
 
 // Tait pressure over rho^2 from rho, fp32, cancellation-free.
 __device__ __forceinline__ float tait_p_over_rho2(float rho, const PhysC &ph)

@@ -31,7 +31,7 @@ def _gpu_rates(w, variant=0, planes=None):
     return out
 
 
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 2])
 def test_config0_rest_state_rates(variant):
     """Prescribed check: config 0 at rest.  p = 0 and v = 0, so every fluid rate is (g, 0)."""
     w = W.dam_break(16)
@@ -44,7 +44,7 @@ def test_config0_rest_state_rates(variant):
     assert np.array_equal(out["pos"], w.pos) and np.array_equal(out["rho"], w.rho)
 
 
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 2])
 @pytest.mark.parametrize("nb", [16, 40])
 def test_scrambled_state_rates(variant, nb):
     """Reading A21: same positions, random velocities and densities, so that pressure,
@@ -70,7 +70,7 @@ def test_variants_agree_and_slabs_do_not_change_rates():
     assert np.array_equal(a["acc"], c["acc"]) and np.array_equal(a["drho"], c["drho"])
 
 
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 2])
 def test_nonuniform_mass_and_cubic_spline(variant):
     w = W.dam_break(12, scrambled=True)
     w.params = dict(w.params)
