@@ -178,8 +178,8 @@ struct IaSmem {
     uint4 hp[IA_NBLK * 6];                    // fp16 filter copy: per block of 16 candidates 2 x uint4 of x, of y,
                                               // of z; half2 word k = (candidate k, candidate k + 8), in units of h
                                               // about the centre of the CTA's neighbourhood
-    uint32_t stack[IA_QCAP * IA_THREADS];     // [entry][thread]: hit mask (bits 0-7: candidates 0-7 of the block,
-                                              // bits 16-23: candidates 8-15) | block index << 8
+    uint32_t stack[IA_QCAP * IA_THREADS];     // [entry][thread]: 16-bit hit mask (bit c = candidate c of the block)
+                                              // | block index << 16
     uint32_t cbt[9][IA_ZMAX + 3];             // cell_begin of the 9 columns over [zlo, zhi]
     uint32_t col_vstart[10];                  // virtual start of each column in the concatenation
     uint32_t stage_lo[9], stage_hi[9];        // global index range of the column staged in this batch
@@ -331,12 +331,11 @@ interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict
             if (cur_mask == 0 && sp > stk_base) {
                 sp -= STK_STRIDE;
                 const uint32_t e = lds_u32(sp);
-                cur_mask = e & 0x00FF00FFu;
-                cur_s = (e & 0xFF00u) >> 4;                          // block index * 16
+                cur_mask = e & 0xFFFFu;                              // bit c = candidate c of the block
+                cur_s = (e >> 12) & 0xFF0u;                          // block index * 16
             }
             ok = cur_mask != 0;
-            const uint32_t bit = (uint32_t)(__ffs(cur_mask) - 1);    // 0..7 or 16..23 (garbage if !ok)
-            s = cur_s + (bit & 7u) + (bit >> 1 & 8u);
+            s = cur_s + (uint32_t)(__ffs(cur_mask) - 1);            // garbage if !ok
             cur_mask &= cur_mask - 1;
         };
         // pair term of candidate s; ok = false turns it into a no-op without a branch (s = 0 is
@@ -466,7 +465,10 @@ interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict
                     if (wide) m = 0x00FF00FFu;
                     if (it == 0) m &= first_mask;
                     if (it == nblk - 1) m &= last_mask;
-                    if (it < nblk && m) { sts_u32(sp, m | (blk << 8)); sp += STK_STRIDE; }
+                    if (it < nblk && m) {                   // entry: linear 16-bit mask | block index << 16
+                        sts_u32(sp, (m & 0xFFu) | ((m >> 8) & 0xFF00u) | (blk << 16));
+                        sp += STK_STRIDE;
+                    }
                     while (__any_sync(lane_full, sp > stk_high)) drain_round();
                 }
             }
@@ -682,12 +684,11 @@ interact_tile_kernel(const float4 *__restrict__ pos4, const float4 *__restrict__
             if (cur_mask == 0 && sp > stk_base) {
                 sp -= STK_STRIDE;
                 const uint32_t e = lds_u32(sp);
-                cur_mask = e & 0x00FF00FFu;
-                cur_s = (e & 0xFF00u) >> 4;                          // block index * 16
+                cur_mask = e & 0xFFFFu;                              // bit c = candidate c of the block
+                cur_s = (e >> 12) & 0xFF0u;                          // block index * 16
             }
             ok = cur_mask != 0;
-            const uint32_t bit = (uint32_t)(__ffs(cur_mask) - 1);    // 0..7 or 16..23 (garbage if !ok)
-            s = cur_s + (bit & 7u) + (bit >> 1 & 8u);
+            s = cur_s + (uint32_t)(__ffs(cur_mask) - 1);            // garbage if !ok
             cur_mask &= cur_mask - 1;
         };
         // pair term of candidate s; ok = false turns it into a no-op without a branch (s = 0 is
@@ -818,7 +819,10 @@ interact_tile_kernel(const float4 *__restrict__ pos4, const float4 *__restrict__
                     if (wide) m = 0x00FF00FFu;
                     if (it == 0) m &= first_mask;
                     if (it == nblk - 1) m &= last_mask;
-                    if (it < nblk && m) { sts_u32(sp, m | (blk << 8)); sp += STK_STRIDE; }
+                    if (it < nblk && m) {                   // entry: linear 16-bit mask | block index << 16
+                        sts_u32(sp, (m & 0xFFu) | ((m >> 8) & 0xFF00u) | (blk << 16));
+                        sp += STK_STRIDE;
+                    }
                     while (__any_sync(lane_full, sp > stk_high)) drain_round();
                 }
             }
