@@ -166,6 +166,7 @@ constexpr int IA_BLK = 16;           // candidates per filter block = per stack 
 constexpr int IA_ZMAX = 32;          // max cells per z-block
 constexpr int IA_CAP = SPH_IA_CAP;   // staged candidates per batch (9 columns x 11 cells x 27 + slack), multiple of 16
 constexpr int IA_NBLK = IA_CAP / IA_BLK;
+constexpr float IA_FAR = 1e15f;      // coordinate of the dummy partner: r2 = 3e30 is finite, F = 0
 constexpr float IA_TINY = 1e-30f;    // r2 floor: a coincident pair (the particle itself) adds exactly 0
 static_assert(IA_CAP % IA_BLK == 0 && IA_NBLK <= 256, "block index must fit 8 bits of a stack entry");
 
@@ -173,8 +174,10 @@ static_assert(IA_CAP % IA_BLK == 0 && IA_NBLK <= 256, "block index must fit 8 bi
 // of an fp32 record - the filter loop is bound by shared-memory bandwidth (ncu: 79 % of the LSU
 // wavefront peak with fp32 records), not by arithmetic.
 struct IaSmem {
-    float4 rel[IA_CAP];                       // exact position relative to the CTA origin; w = p/rho^2
-    float4 vr[IA_CAP];                        // vx, vy, vz, rho (sign bit = boundary type if masses differ)
+    float4 rel[IA_CAP + 1];                   // exact position relative to the CTA origin; w = p/rho^2
+    float4 vr[IA_CAP + 1];                    // vx, vy, vz, rho (sign bit = boundary type if masses differ)
+                                              // slot IA_CAP of both: a particle at rest far outside every
+                                              // support, the partner of drain slots that have no pair
     uint4 hp[IA_NBLK * 6];                    // fp16 filter copy: per block of 16 candidates 2 x uint4 of x, of y,
                                               // of z; half2 word k = (candidate k, candidate k + 8), in units of h
                                               // about the centre of the CTA's neighbourhood
@@ -263,7 +266,11 @@ interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict
 
     const int zlo = max(cz0 - 1, 0), zhi = min(cz1 + 1, g.nc[2]);
     const int nz = zhi - zlo;                                    // <= zb + 2
-    if (tid == 0) s_wide = 0u;
+    if (tid == 0) {
+        s_wide = 0u;
+        S.rel[IA_CAP] = make_float4(IA_FAR, IA_FAR, IA_FAR, 0.f);
+        S.vr[IA_CAP] = make_float4(0.f, 0.f, 0.f, 1.f);
+    }
     // ---- cell-begin table of the 9 columns
     for (int k = tid; k < 9 * (nz + 1); k += IA_THREADS) {
         int col = k / (nz + 1), z = k % (nz + 1);
@@ -338,19 +345,19 @@ interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict
             s = cur_s + (uint32_t)(__ffs(cur_mask) - 1);            // garbage if !ok
             cur_mask &= cur_mask - 1;
         };
-        // pair term of candidate s; ok = false turns it into a no-op without a branch (s = 0 is
-        // always a staged, finite candidate; its mass factor is zeroed).  The exact fp32 distance is
+        // pair term of candidate s; ok = false turns it into a no-op without a branch: the partner is
+        // the far-away dummy slot, whose F is 0.  The exact fp32 distance is
         // formed here: a candidate the fp16 filter let through although it lies outside 2h adds
         // exactly 0 because F is clamped.
         auto interact = [&](uint32_t s, bool ok) {
-            s = ok ? s : 0u;
+            s = ok ? s : (uint32_t)IA_CAP;
             const float4 rj = lds_f4(rel_base + 16u * s);
             float4 vj = lds_f4(rel_base + vr_delta + 16u * s);
             const float dx = xi - rj.x, dy = yi - rj.y, dz = zi - rj.z;     // == absolute differences
             const float r2 = fmaxf(fmaf(dz, dz, fmaf(dy, dy, dx * dx)), IA_TINY);
-            float mj = ok ? 1.0f : 0.0f;
+            float mj = 1.0f;
             if (!UNIFORM) {
-                mj = ok ? (vj.w < 0.f ? ph.mass_bound : ph.mass_fluid) : 0.0f;
+                mj = vj.w < 0.f ? ph.mass_bound : ph.mass_fluid;
                 vj.w = fabsf(vj.w);
             }
             pair_term<KERNEL, GAMMA7, MU>(dx, dy, dz, r2, vi.x, vi.y, vi.z, vi.w, pi.w, ci, vj, rj.w, mj, ph,
@@ -541,8 +548,8 @@ constexpr int TI_NBLK = TI_CAP / IA_BLK;
 static_assert(TI_CAP % IA_BLK == 0 && TI_NBLK <= 256, "block index must fit 8 bits of a stack entry");
 
 struct TiSmem {
-    float4 rel[TI_CAP];
-    float4 vr[TI_CAP];
+    float4 rel[TI_CAP + 1];
+    float4 vr[TI_CAP + 1];
     uint4 hp[TI_NBLK * 6];
     uint32_t stack[TI_QCAP * TI_THREADS];
     uint32_t cbt[TI_COL][TI_ZMAX + 3];
@@ -593,7 +600,11 @@ interact_tile_kernel(const float4 *__restrict__ pos4, const float4 *__restrict__
         }
         if (any == 0) return;
     }
-    if (tid == 0) s_wide = 0u;
+    if (tid == 0) {
+        s_wide = 0u;
+        S.rel[TI_CAP] = make_float4(IA_FAR, IA_FAR, IA_FAR, 0.f);
+        S.vr[TI_CAP] = make_float4(0.f, 0.f, 0.f, 1.f);
+    }
     // ---- target ranges of the TI_B x TI_B own columns, concatenated
     if (tid < TI_B * TI_B) {
         const int x = cx0 + tid / TI_B, y = cy0 + tid % TI_B;
@@ -691,19 +702,19 @@ interact_tile_kernel(const float4 *__restrict__ pos4, const float4 *__restrict__
             s = cur_s + (uint32_t)(__ffs(cur_mask) - 1);            // garbage if !ok
             cur_mask &= cur_mask - 1;
         };
-        // pair term of candidate s; ok = false turns it into a no-op without a branch (s = 0 is
-        // always a staged, finite candidate; its mass factor is zeroed).  The exact fp32 distance is
+        // pair term of candidate s; ok = false turns it into a no-op without a branch: the partner is
+        // the far-away dummy slot, whose F is 0.  The exact fp32 distance is
         // formed here: a candidate the fp16 filter let through although it lies outside 2h adds
         // exactly 0 because F is clamped.
         auto interact = [&](uint32_t s, bool ok) {
-            s = ok ? s : 0u;
+            s = ok ? s : (uint32_t)TI_CAP;
             const float4 rj = lds_f4(rel_base + 16u * s);
             float4 vj = lds_f4(rel_base + vr_delta + 16u * s);
             const float dx = xi - rj.x, dy = yi - rj.y, dz = zi - rj.z;     // == absolute differences
             const float r2 = fmaxf(fmaf(dz, dz, fmaf(dy, dy, dx * dx)), IA_TINY);
-            float mj = ok ? 1.0f : 0.0f;
+            float mj = 1.0f;
             if (!UNIFORM) {
-                mj = ok ? (vj.w < 0.f ? ph.mass_bound : ph.mass_fluid) : 0.0f;
+                mj = vj.w < 0.f ? ph.mass_bound : ph.mass_fluid;
                 vj.w = fabsf(vj.w);
             }
             pair_term<KERNEL, GAMMA7, MU>(dx, dy, dz, r2, vi.x, vi.y, vi.z, vi.w, pi.w, ci, vj, rj.w, mj, ph,
