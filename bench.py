@@ -35,8 +35,8 @@ METRIC = "Mparticle-steps/s"
 FP32_LANES_PER_SM, NUM_SMS = 128, 148
 FLOPS_PER_CANDIDATE, FLOPS_PER_PAIR = 8, 32
 # dram__bytes_read.sum + dram__bytes_write.sum of one interact_staged_kernel launch at config 3
-# (profiles/r01_ncu_full_config3_v3.md); other configs have no capture
-IA_TRAFFIC_BYTES = {3: 1.382216e9 + 0.530205e9}
+# (profiles/r01_ncu_full_config3_v4.md); other configs have no capture
+IA_TRAFFIC_BYTES = {3: 1.379577e9 + 0.529622e9}
 # algorithmic HBM bytes per particle of the memory-bound stages
 BYTES = dict(keys=28.0, sort_per_pass=16.0, gather=116.0, verlet=116.0, migrate=4.0)
 
