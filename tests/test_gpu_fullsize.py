@@ -46,3 +46,28 @@ def test_config3_full_size_structure_and_sampled_rates():
         scale_d = max(scale_d, abs(d[k]))
     assert scale_a > 0 and scale_d > 0
     assert worst_a <= 1e-4 * scale_a and worst_d <= 1e-4 * scale_d
+
+
+def test_config1_full_size_ten_steps():
+    """BASELINE config 1 (1.2 M particles, 3 slabs rebuilt every step) at full size: state after 10
+    Verlet steps against ORACLE B stepping the same 10 steps in fp64 (north star: relative L2 <= 1e-3)."""
+    from gpu_util import rel_l2
+    w = W.dam_break(100, scrambled=True, n_slabs=3)
+    nc = OA.grid_dims(w.params["dom_min"], w.params["dom_max"], w.params["h"])
+    sph = make_sph(w)
+    sph.sph_set_slabs(W.slab_planes(nc[0], 3))
+    p = OB.params_from_workload(w.params)
+    s = OB.State(w.pos, w.vel, w.rho, w.type)
+    for _ in range(10):
+        sph.sph_step(w.dt)
+        OB.step(p, s, w.dt, verlet_ns=w.params["verlet_ns"])
+    out = sph.sph_download()
+    assert sph.sph_status() == 0
+    fl = w.type == 0
+    assert rel_l2(out["pos"], s.r) <= 1e-3
+    assert rel_l2(out["rho"], s.rho) <= 1e-3
+    assert rel_l2(out["vel"][fl], s.v[fl]) <= 1e-3
+    disp_ref = s.r[fl] - w.pos[fl].astype(np.float64)
+    disp = out["pos"][fl].astype(np.float64) - w.pos[fl].astype(np.float64)
+    assert np.linalg.norm(disp - disp_ref) <= 1e-3 * np.linalg.norm(disp_ref)
+    assert np.array_equal(out["pos"][~fl], w.pos[~fl])
