@@ -8,7 +8,7 @@ Mparticle-steps/s on synthetic 3-D dam breaks, radix-sort Gkeys/s, % of roofline
 One "step" = one sph_step() = all rows of the hot path (keys+tags, radix sort, payload
 permutation, cell table, halo gather, migrant compaction, 27-cell interaction, Verlet) over the
 whole particle set.  Default workload: BASELINE config 3 (32 M fluid + 2 M boundary particles,
-16 logical x-slabs), the size the roofline bars are judged at; its working set (6.5 GB) is far
+16 logical x-slabs), the size the roofline bars are judged at; its working set (6.7 GB) is far
 larger than the 126 MB L2, so no L2 flush is needed between steps.
 
 N > 1 (torchrun): the path has no inter-GPU exchange (BASELINE north_star drops it), so every
@@ -407,7 +407,7 @@ def main():
                              f"particles, {w.n_slabs} logical x-slabs",
                     n_particles=n, n_slabs=w.n_slabs, cells=int(v.ncells), cell_bits=int(v.cell_bits),
                     radix_passes=passes, dt=("variable, cfl 0.2" if args.adaptive else w.dt), multi_gpu="replicas only",
-                    l2="no flush: per-step working set %.1f GB >> 126 MB L2" % (n * 250e-9)
+                    l2="no flush: per-step working set %.1f GB >> 126 MB L2" % (n * 198e-9)
                     if n > 5_000_000 else "working set fits L2 (small config)"),
         clocks=clocks, e2e=e2e, gpu_launches=int(launches), roofline=roofline, cpu_baseline=cpu,
         sort_gkeys_s=n / (stages["sort"]["ms"] * 1e-3) / 1e9 if "sort" in stages else None,
