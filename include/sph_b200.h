@@ -158,6 +158,16 @@ int sph_build_halos(sph_ctx *ctx, const int32_t *planes, int n_slabs);
 /* a7: acc4 = (dv/dt, d rho/dt) of every particle.  Needs the cell table. */
 int sph_interact(sph_ctx *ctx);
 
+/* a7 for ONE logical sub-domain, the way GPU_k does it in the paper (L192, L218-220, L226-228): the
+ * rates of the particles slab `slab` owns, computed from its own particles and the two HALO BUFFERS
+ * that sph_build_halos filled, and from nothing else - the local set is assembled, its cell table is
+ * rebuilt from the particles' positions, and the production interaction kernel runs on it.  Results go
+ * to the slab's range of acc4; calling it for every slab reproduces sph_interact value for value (the
+ * device-side proof that a 2h halo suffices).  Needs sph_build_halos since the last sort (else
+ * SPH_ERR_ORDER); uses the idle halves of the state buffers as scratch; synchronises the stream once
+ * (the slab ranges cross to the host). */
+int sph_interact_slab(sph_ctx *ctx, int slab);
+
 /* a1-a8 in order; dt > 0. */
 int sph_step(sph_ctx *ctx, float dt);
 

@@ -29,7 +29,7 @@ SPH_OPT_INTERACT_VARIANT = 0
 SPH_OPT_ADAPTIVE_DT = 1
 
 EXPORTS = ["sph_workspace_bytes", "sph_init", "sph_set_state", "sph_set_slabs", "sph_slab_planes_from_x",
-           "sph_sort_and_cells", "sph_build_halos", "sph_interact", "sph_step", "sph_time_step", "sph_step_adaptive", "sph_get_view",
+           "sph_sort_and_cells", "sph_build_halos", "sph_interact", "sph_interact_slab", "sph_step", "sph_time_step", "sph_step_adaptive", "sph_get_view",
            "sph_download", "sph_status", "sph_set_option", "sph_profile_enable", "sph_profile_read",
            "sph_pair_stats", "sph_launch_count", "sph_destroy", "sph_strerror"]
 
@@ -71,6 +71,8 @@ _lib.sph_slab_planes_from_x.argtypes = [C.c_void_p, C.POINTER(C.c_float), C.c_in
 for _name in ("sph_sort_and_cells", "sph_interact", "sph_status"):
     getattr(_lib, _name).restype = C.c_int
     getattr(_lib, _name).argtypes = [C.c_void_p]
+_lib.sph_interact_slab.restype = C.c_int
+_lib.sph_interact_slab.argtypes = [C.c_void_p, C.c_int]
 _lib.sph_build_halos.restype = C.c_int
 _lib.sph_build_halos.argtypes = [C.c_void_p, C.POINTER(C.c_int32), C.c_int]
 _lib.sph_step.restype = C.c_int
@@ -220,6 +222,9 @@ class Sph:
 
     def sph_interact(self):
         _check(_lib.sph_interact(self._ctx))
+
+    def sph_interact_slab(self, slab: int):
+        _check(_lib.sph_interact_slab(self._ctx, int(slab)))
 
     def sph_step(self, dt: float):
         _check(_lib.sph_step(self._ctx, float(dt)))

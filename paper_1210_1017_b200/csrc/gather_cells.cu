@@ -17,24 +17,6 @@
 
 namespace sph {
 
-constexpr uint32_t GAP_INLINE = 32;        // cells a thread fills itself
-constexpr uint32_t GAP_CHUNK = 1u << 16;   // cells per work-list entry
-
-__device__ __forceinline__ void fill_cells(uint32_t lo, uint32_t hi /* inclusive */, uint32_t value,
-                                           uint32_t *__restrict__ cell_begin, uint4 *__restrict__ gap_list,
-                                           uint32_t *__restrict__ gap_count)
-{
-    if (hi - lo < GAP_INLINE) {
-        for (uint32_t cc = lo; cc <= hi; ++cc) cell_begin[cc] = value;
-    } else {
-        for (uint32_t a = lo; a <= hi; a += GAP_CHUNK) {
-            const uint32_t b = min(hi, a + (GAP_CHUNK - 1u));
-            gap_list[atomicAdd(gap_count, 1u)] = make_uint4(a, b, value, 0u);
-            if (b == hi) break;              // a + GAP_CHUNK could wrap for hi near 2^32
-        }
-    }
-}
-
 __global__ void __launch_bounds__(GATHER_THREADS)
 gather_kernel(uint32_t n, uint32_t ncells, const uint2 *__restrict__ kv,
               const float4 *__restrict__ pos_in, const float4 *__restrict__ vr_in,
@@ -117,12 +99,17 @@ cudaError_t launch_gather_cells(sph_ctx *c)
 }
 
 // long gaps of the cell table (work list written by gather_kernel)
+cudaError_t launch_gap_fill(sph_ctx *c, uint32_t *table)
+{
+    gap_fill_kernel<<<NUM_SMS * 4, 256, 0, c->stream>>>(c->gap_list, c->counters + 8, table);
+    c->n_launches++;
+    return cudaGetLastError();
+}
+
 cudaError_t launch_cell_fill(sph_ctx *c)
 {
     if (c->n == 0) return cudaSuccess;
-    gap_fill_kernel<<<NUM_SMS * 4, 256, 0, c->stream>>>(c->gap_list, c->counters + 8, c->cell_begin);
-    c->n_launches++;
-    return cudaGetLastError();
+    return launch_gap_fill(c, c->cell_begin);
 }
 
 // ---- slab ranges, halo ranges and offsets -------------------------------------------------------

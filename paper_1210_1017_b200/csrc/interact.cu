@@ -246,7 +246,8 @@ interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict
                        const uint32_t *__restrict__ idt, const uint32_t *__restrict__ keyword,
                        const uint32_t *__restrict__ cell_begin, float4 *__restrict__ acc4, float *__restrict__ mu_out,
                        GridC g, PhysC ph, int zb, int nzb, float thr_h /* filter threshold, units of h^2 */,
-                       float zlim /* |z| bound the threshold was derived for, units of h */)
+                       float zlim /* |z| bound the threshold was derived for, units of h */,
+                       int cx_first /* first cell plane of the targets (per-slab execution), else 0 */)
 {
     extern __shared__ __align__(16) unsigned char ia_raw[];
     IaSmem &S = *reinterpret_cast<IaSmem *>(ia_raw);
@@ -258,7 +259,7 @@ interact_staged_kernel(const float4 *__restrict__ pos4, const float4 *__restrict
     const int bz = b % nzb;
     b /= nzb;
     const int cy = b % g.nc[1];
-    const int cx = b / g.nc[1];
+    const int cx = b / g.nc[1] + cx_first;
     const int cz0 = bz * zb, cz1 = min(cz0 + zb, g.nc[2]);
     const uint32_t own_col = (uint32_t)(cx * g.nc[1] + cy) * g.nc[2];
     const uint32_t t_begin = cell_begin[own_col + cz0], t_end = cell_begin[own_col + cz1];
@@ -520,12 +521,16 @@ static cudaError_t launch_staged(sph_ctx *c)
     }
     int zb = c->zblock;
     int nzb = (c->grid.nc[2] + zb - 1) / zb;
-    uint64_t blocks = (uint64_t)c->grid.nc[0] * c->grid.nc[1] * nzb;
+    const IaOverride &ov = c->ia_ov;               // per-slab execution works on a local particle set
+    const int cx_first = ov.on ? ov.cx_first : 0, cx_count = ov.on ? ov.cx_count : c->grid.nc[0];
+    uint64_t blocks = (uint64_t)cx_count * c->grid.nc[1] * nzb;
+    if (blocks == 0) return cudaSuccess;
     float thr_h, zlim;
     filter_threshold(zb, &thr_h, &zlim);
     kern<<<(uint32_t)blocks, IA_THREADS, sizeof(IaSmem) + SPH_IA_PAD, c->stream>>>(
-        c->pos4[c->cur], c->velrho4[c->cur], c->idt[c->cur], c->keyword, c->cell_begin, c->acc4, c->mumax,
-        c->grid, c->phys, zb, nzb, thr_h, zlim);
+        ov.on ? ov.pos4 : c->pos4[c->cur], ov.on ? ov.velrho4 : c->velrho4[c->cur], ov.on ? ov.idt : c->idt[c->cur],
+        ov.on ? ov.keyword : c->keyword, ov.on ? ov.cell_begin : c->cell_begin, ov.on ? ov.acc4 : c->acc4, c->mumax,
+        c->grid, c->phys, zb, nzb, thr_h, zlim, cx_first);
     c->n_launches++;
     return cudaGetLastError();
 }

@@ -46,14 +46,6 @@ cudaError_t launch_init_state(sph_ctx *c, const float *pos, const float *vel, co
 }
 
 // ---- keys -----------------------------------------------------------------------------------
-__device__ __forceinline__ int cell_coord(float x, float mn, float inv, int nc)
-{
-    // one separately rounded fp32 subtract, one fp32 multiply, floor, clamp
-    float t = __fmul_rn(__fsub_rn(x, mn), inv);
-    int ci = __float2int_rd(t);           // floor; saturates for huge |t|
-    return min(max(ci, 0), nc - 1);
-}
-
 // Largest s with table[s] <= x, for a shared-memory table of 17 ascending entries padded with
 // "infinity" beyond the used ones (4 probes instead of a 15-way compare chain).
 template <typename T>

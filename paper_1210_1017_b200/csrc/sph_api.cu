@@ -16,7 +16,7 @@ size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 
 struct Layout {
     size_t pos4[2], velrho4[2], velrhoM1[2], idt[2], acc4, mumax, dt_red, kv[2], keyword, hist, tile_state, counters,
-        cell_begin, gap_list, mig_tile, mig_grp, mig_off, scratch64, slab_begin, halo_range, halo_offset, halo_pos4, halo_velrho4, halo_idt,
+        cell_begin, cell_loc, gap_list, mig_tile, mig_grp, mig_off, scratch64, slab_begin, halo_range, halo_offset, halo_pos4, halo_velrho4, halo_idt,
         migrants, mig_total, mig_count, prev_init, flags, total;
 };
 
@@ -64,6 +64,7 @@ bool make_layout(const sph_params *p, uint64_t n, int max_slabs, Layout *L)
     L->tile_state = take((size_t)4 * 256 * tiles * 4);
     L->counters = take(4 * 64);
     L->cell_begin = take(4 * (ncells + 1));
+    L->cell_loc = take(max_slabs > 1 ? 4 * (ncells + 1) : 4);
     L->gap_list = take(16 * gap_list_entries(ncells));
     L->mig_tile = take(4 * ((size_t)gather_tiles(nn) + 1));
     L->mig_grp = take(4 * ((size_t)mig_groups(nn) + 1));
@@ -277,6 +278,8 @@ int sph_init(sph_ctx **out, const sph_params *p, const sph_particles *part, int 
     c->counters = (uint32_t *)(w + L.counters);
     c->rs_tiles = radix_tiles(c->n);
     c->cell_begin = (uint32_t *)(w + L.cell_begin);
+    c->cell_loc = (uint32_t *)(w + L.cell_loc);
+    c->ia_ov.on = false;
     c->gap_list = (uint4 *)(w + L.gap_list);
     c->mig_tile = (uint32_t *)(w + L.mig_tile);
     c->mig_grp = (uint32_t *)(w + L.mig_grp);
@@ -446,6 +449,30 @@ int sph_step(sph_ctx *c, float dt)
     rc = sph_interact(c);
     if (rc != SPH_OK) return rc;
     return verlet_and_advance(c, dt);
+}
+
+int sph_interact_slab(sph_ctx *c, int slab)
+{
+    if (!c) return SPH_ERR_ARG;
+    if (c->sticky) return c->sticky;
+    if (!c->sorted_valid || !c->halos_valid) return SPH_ERR_ORDER;
+    const int S = c->tagged_slabs.n_slabs;
+    if (slab < 0 || slab >= S) return SPH_ERR_ARG;
+    if (c->max_slabs < 2 && S > 1) return SPH_ERR_ARG;
+    uint32_t h_begin[SPH_MAX_SLABS + 1], h_range[4 * SPH_MAX_SLABS], h_off[2 * SPH_MAX_SLABS + 1];
+    memset(h_range, 0, sizeof(h_range));
+    memset(h_off, 0, sizeof(h_off));
+    CK(c, cudaMemcpyAsync(h_begin, c->slab_begin, 4 * (S + 1), cudaMemcpyDeviceToHost, c->stream));
+    if (S > 1) {
+        CK(c, cudaMemcpyAsync(h_range, c->halo_range, 4 * 4 * S, cudaMemcpyDeviceToHost, c->stream));
+        CK(c, cudaMemcpyAsync(h_off, c->halo_offset, 4 * (2 * S + 1), cudaMemcpyDeviceToHost, c->stream));
+    }
+    CK(c, cudaStreamSynchronize(c->stream));
+    Timed t(c, SPH_T_INTERACT);
+    CK(c, launch_interact_slab(c, slab, h_begin, h_range, h_off));
+    c->rates_valid = true;
+    c->mu_valid = false;
+    return SPH_OK;
 }
 
 int sph_time_step(sph_ctx *c, float cfl, float *dt, float *amax_slab, float *smax_slab)

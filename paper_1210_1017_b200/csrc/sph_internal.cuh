@@ -47,6 +47,16 @@ struct PhysC {
     int kernel;
 };
 
+// ---- per-slab execution: arrays and cell planes the interaction kernel works on instead of the
+// context's own (sph_interact_slab, slab_exec.cu) ----------------------------------------------
+struct IaOverride {
+    bool on;
+    const float4 *pos4, *velrho4;
+    const uint32_t *idt, *keyword, *cell_begin;
+    float4 *acc4;
+    int cx_first, cx_count;      // cell planes [cx_first, cx_first + cx_count) hold the targets
+};
+
 // ---- profiling ------------------------------------------------------------------------
 struct StageTimer {
     static constexpr int MAX_PAIRS = 16384;
@@ -118,6 +128,8 @@ struct sph_ctx {
     uint64_t n_launches;       // kernels launched so far (memsets and copies not counted)
 
     sph::StageTimer timer;
+    sph::IaOverride ia_ov;     // off except inside sph_interact_slab
+    uint32_t *cell_loc;        // ncells+1: cell table a slab rebuilds from its own + halo particles
 };
 
 namespace sph {
@@ -135,6 +147,9 @@ cudaError_t launch_halo_gather(sph_ctx *c);
 cudaError_t launch_migrants(sph_ctx *c);
 cudaError_t launch_interact(sph_ctx *c, bool with_mu);
 cudaError_t launch_dt_reduce(sph_ctx *c);
+cudaError_t launch_gap_fill(sph_ctx *c, uint32_t *table);
+cudaError_t launch_interact_slab(sph_ctx *c, int slab, const uint32_t *h_slab_begin, const uint32_t *h_halo_range,
+                                 const uint32_t *h_halo_offset);
 cudaError_t launch_verlet(sph_ctx *c, float dt, int corrective);
 cudaError_t launch_pair_stats(sph_ctx *c, unsigned long long *d_out);
 cudaError_t launch_download_pack(sph_ctx *c, float *pos3, float *vel3, float *rho, float *acc3,
@@ -157,6 +172,34 @@ __device__ __forceinline__ float tait_p_over_rho2(float rho, const PhysC &ph)
     for (int k = ph.gamma - 1; k >= 1; --k) s = fmaf(s, d, ph.tait[k]);
     float p = ph.B * d * s;
     return __fdividef(p, rho * rho);
+}
+
+// Cell coordinate along one axis: one separately rounded fp32 subtract, one fp32 multiply, floor,
+// clamp - the sequence ORACLE A pins (a1).
+__device__ __forceinline__ int cell_coord(float x, float mn, float inv, int nc)
+{
+    float t = __fmul_rn(__fsub_rn(x, mn), inv);
+    int ci = __float2int_rd(t);           // floor; saturates for huge |t|
+    return min(max(ci, 0), nc - 1);
+}
+
+// cell_begin[lo..hi] = value: short gaps by the calling thread, long ones through the work list that
+// gap_fill_kernel empties (gather_cells.cu).
+constexpr uint32_t GAP_INLINE = 32;        // cells a thread fills itself
+constexpr uint32_t GAP_CHUNK = 1u << 16;   // cells per work-list entry
+__device__ __forceinline__ void fill_cells(uint32_t lo, uint32_t hi /* inclusive */, uint32_t value,
+                                           uint32_t *__restrict__ cell_begin, uint4 *__restrict__ gap_list,
+                                           uint32_t *__restrict__ gap_count)
+{
+    if (hi - lo < GAP_INLINE) {
+        for (uint32_t cc = lo; cc <= hi; ++cc) cell_begin[cc] = value;
+    } else {
+        for (uint32_t a = lo; a <= hi; a += GAP_CHUNK) {
+            const uint32_t b = min(hi, a + (GAP_CHUNK - 1u));
+            gap_list[atomicAdd(gap_count, 1u)] = make_uint4(a, b, value, 0u);
+            if (b == hi) break;              // a + GAP_CHUNK could wrap for hi near 2^32
+        }
+    }
 }
 
 // Warps with at most this many runs of equal digits use the hardware MATCH.ANY (about 8 cycles per
