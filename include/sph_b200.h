@@ -119,9 +119,9 @@ enum {
 
 /* Options for sph_set_option. */
 enum {
-    SPH_OPT_INTERACT_VARIANT = 0, /* 0 = smem-staged production kernel, 1 = simple
-                                     one-thread-per-particle kernel (cross-check), 2 = staged
-                                     kernel over tiles of 2 x 2 columns (cross-check) */
+    SPH_OPT_INTERACT_VARIANT = 0, /* 0 = production kernel, 1 = simple one-thread-per-particle
+                                     kernel (cross-check), 2 = the round-1 staged kernel with the
+                                     fp16 ALU filter (cross-check) */
     SPH_OPT_ADAPTIVE_DT = 1       /* 1 = sph_interact also records max_j |mu_ij| of every particle,
                                      which sph_time_step needs (costs a few instructions per pair);
                                      0 (default) = fixed-dt path */
@@ -188,14 +188,42 @@ int sph_time_step(sph_ctx *ctx, float cfl, float *dt, float *amax_slab, float *s
  * the paper's does for its MPI_Allreduce). */
 int sph_step_adaptive(sph_ctx *ctx, float cfl, float *dt_used);
 
+/* Movable slab planes (dynamic load balancing; "a multidimensional domain decomposition
+ * with load balancing", L389).  From the per-plane particle counts that the cell table of the last
+ * sort holds, choose planes_out[0..n_slabs] (HOST int32) so that the slabs own about n / n_slabs
+ * particles each: plane s = the cell plane p in [planes[s-1] + 2, ncx - 2 (n_slabs - s)] that minimises
+ * |#(particles left of p) * n_slabs - s * n|, the lowest such p on ties, chosen left to right (every
+ * slab keeps >= 2 cell planes, reading A14).  Does not change the context: hand the planes to
+ * sph_build_halos(planes) (new owners, edge labels, halos and migrants without a new sort: a particle
+ * whose owner changes because a plane moved is a migrant, reading A15) or to sph_set_slabs.  Needs a sort
+ * since the last state change; synchronises the stream.  SPH_ERR_SLABS if nc[0] < 2 n_slabs. */
+int sph_balance_slabs(sph_ctx *ctx, int n_slabs, int32_t *planes_out);
+
+/* The borrowed device pointers of the current state ("data is stored on the GPU
+ * memory"; everything a4-a6 produce stays there for the next stage, L224-228). */
 int sph_get_view(sph_ctx *ctx, sph_view *out);
 
-/* HOST outputs in ID order, any of them may be NULL: pos n*3, vel n*3, rho n, acc n*3, drho n.
- * Synchronises the stream. */
+/* Saving results (particle data "are copied to the host only when saving", L211-212
+ * "copy all particle data to host").  HOST outputs in ID order, any of them may be NULL: pos n*3,
+ * vel n*3, rho n, acc n*3, drho n.  Synchronises the stream. */
 int sph_download(sph_ctx *ctx, float *pos, float *vel, float *rho, float *acc, float *drho);
 
-/* Synchronise the stream; return the sticky error (SPH_OK, SPH_ERR_CUDA, SPH_ERR_NONFINITE). */
+/* Exact checkpoint / resume (same passages): the part of the state sph_download does not return - the
+ * Verlet n-1 velocity and density (reading A7) in ID order, HOST vel_m1 n*3 and rho_m1 n (may be NULL),
+ * and the number of completed steps.  To resume: sph_init / sph_set_state with the saved pos, vel, rho,
+ * then sph_set_resume (HOST or DEVICE arrays, on_device says which) BEFORE the next sort (else
+ * SPH_ERR_ORDER); the run then continues bit for bit as if it had never stopped (the sort order is
+ * history-free, reading A12).  Both synchronise the stream (sph_set_resume only for HOST inputs). */
+int sph_download_resume(sph_ctx *ctx, float *vel_m1, float *rho_m1, uint64_t *step_index);
+int sph_set_resume(sph_ctx *ctx, const float *vel_m1, const float *rho_m1, uint64_t step_index, int on_device);
+
+/* Synchronise the stream; return the sticky error (SPH_OK, SPH_ERR_CUDA, SPH_ERR_NONFINITE: the device
+ * flag raised by any kernel that met a non-finite position, velocity, density or rate). */
 int sph_status(sph_ctx *ctx);
+
+/* Text of the last failed CUDA runtime call of this context (ctx = NULL: of the calling thread, for
+ * failures inside sph_init); "" if none.  The library never prints. */
+const char *sph_last_cuda_error(const sph_ctx *ctx);
 
 int sph_set_option(sph_ctx *ctx, int option, int value);
 
@@ -212,6 +240,12 @@ int sph_profile_read(sph_ctx *ctx, float *ms, int *launches);
  * sph_launch_count: HOST *out = number of kernels this context has launched so far. */
 int sph_pair_stats(sph_ctx *ctx, uint64_t *out);
 int sph_launch_count(const sph_ctx *ctx, uint64_t *out);
+
+/* Measured FP32 peak of this GPU: a register-resident chain of fused multiply-adds,
+ * variant 0 = scalar FFMA, 1 = packed FFMA2 (two fp32 lanes per instruction); iters >= 1 rounds of 64
+ * FMA lanes per thread on 148 x 8 CTAs of 256 threads; HOST *tflops = 2 flop per FMA / CUDA-event time.
+ * The denominator bench.py reports beside the nominal 148 x 128 x 2 x clock.  Synchronises. */
+int sph_fma_peak(sph_ctx *ctx, int variant, int iters, double *tflops);
 
 void sph_destroy(sph_ctx *ctx);
 const char *sph_strerror(int code);

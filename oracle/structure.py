@@ -24,6 +24,8 @@ Readings where the paper is silent (DESIGN.md section "Readings", SURVEY.md 8(c)
 cells are linearised x-major / z-fastest; indices are clamped to the grid; slabs are
 aligned to cell planes; the first call has no migrants.
 
+Movable planes: ``balance_planes`` (equalise the owned counts, >= 2 planes per slab).
+
 Pins (tests/test_oracle_structure.py): the paper's printed sort example L242-260
 (tests/golden/paper_halo_sort_example.txt); hand-placed particles with exactly
 representable coordinates; brute-force set definitions; halo sufficiency against
@@ -131,6 +133,40 @@ def cell_table(sorted_cells, ncells):
     begin = np.searchsorted(sorted_cells, c, side="left").astype(np.uint32)
     end = np.searchsorted(sorted_cells, c, side="right").astype(np.uint32)
     return begin, end
+
+
+def plane_counts(pos32, dom_min, dom_max, h):
+    """Number of particles in every cell plane along x (bincount of cx)."""
+    nc = grid_dims(dom_min, dom_max, h)
+    cx, _, _ = cell_coords(pos32, dom_min, h, nc)
+    return np.bincount(cx, minlength=nc[0]).astype(np.int64)
+
+
+def balance_planes(counts, n_slabs):
+    """Movable slab planes (PAPER.md L184 "domain decomposition with load balancing", L389;
+    SURVEY 8(f) NEXT-4; reading A22): from the per-plane particle counts choose
+    planes[0..S] so that every slab owns about N/S particles.  With C[p] = particles in planes
+    < p, plane s (s = 1..S-1, left to right) is the p in [planes[s-1] + 2, ncx - 2 (S - s)]
+    that minimises |C[p] S - s N| (exact integers), the lowest p on ties; every slab keeps
+    at least two cell planes (edge = one plane on each side, reading A14)."""
+    counts = [int(c) for c in counts]
+    ncx, S = len(counts), int(n_slabs)
+    assert S == 1 or ncx >= 2 * S
+    C = [0]
+    for c in counts:
+        C.append(C[-1] + c)
+    N = C[-1]
+    planes = [0]
+    for s in range(1, S):
+        lo, hi = planes[-1] + 2, ncx - 2 * (S - s)
+        best, best_cost = None, None
+        for p in range(lo, hi + 1):                     # plain argmin, first minimum wins
+            cost = abs(C[p] * S - s * N)
+            if best is None or cost < best_cost:
+                best, best_cost = p, cost
+        planes.append(best)
+    planes.append(ncx)
+    return planes
 
 
 def structure(pos32, ids, dom_min, dom_max, h, planes, prev_slab=None):

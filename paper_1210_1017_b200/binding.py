@@ -31,7 +31,8 @@ SPH_OPT_ADAPTIVE_DT = 1
 EXPORTS = ["sph_workspace_bytes", "sph_init", "sph_set_state", "sph_set_slabs", "sph_slab_planes_from_x",
            "sph_sort_and_cells", "sph_build_halos", "sph_interact", "sph_interact_slab", "sph_step", "sph_time_step", "sph_step_adaptive", "sph_get_view",
            "sph_download", "sph_status", "sph_set_option", "sph_profile_enable", "sph_profile_read",
-           "sph_pair_stats", "sph_launch_count", "sph_destroy", "sph_strerror"]
+           "sph_pair_stats", "sph_launch_count", "sph_destroy", "sph_strerror", "sph_balance_slabs",
+           "sph_download_resume", "sph_set_resume", "sph_last_cuda_error", "sph_fma_peak"]
 
 
 class sph_params(C.Structure):
@@ -96,6 +97,16 @@ _lib.sph_pair_stats.restype = C.c_int
 _lib.sph_pair_stats.argtypes = [C.c_void_p, C.POINTER(C.c_uint64)]
 _lib.sph_launch_count.restype = C.c_int
 _lib.sph_launch_count.argtypes = [C.c_void_p, C.POINTER(C.c_uint64)]
+_lib.sph_balance_slabs.restype = C.c_int
+_lib.sph_balance_slabs.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_int32)]
+_lib.sph_download_resume.restype = C.c_int
+_lib.sph_download_resume.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_uint64)]
+_lib.sph_set_resume.restype = C.c_int
+_lib.sph_set_resume.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint64, C.c_int]
+_lib.sph_last_cuda_error.restype = C.c_char_p
+_lib.sph_last_cuda_error.argtypes = [C.c_void_p]
+_lib.sph_fma_peak.restype = C.c_int
+_lib.sph_fma_peak.argtypes = [C.c_void_p, C.c_int, C.c_int, C.POINTER(C.c_double)]
 _lib.sph_destroy.restype = None
 _lib.sph_destroy.argtypes = [C.c_void_p]
 _lib.sph_strerror.restype = C.c_char_p
@@ -103,9 +114,9 @@ _lib.sph_strerror.argtypes = [C.c_int]
 
 
 class SphError(RuntimeError):
-    def __init__(self, code: int):
+    def __init__(self, code: int, detail: str = ""):
         self.code = code
-        super().__init__(f"libsph_b200: {sph_strerror(code)} ({code})")
+        super().__init__(f"libsph_b200: {sph_strerror(code)} ({code})" + (f": {detail}" if detail else ""))
 
 
 def sph_strerror(code: int) -> str:
@@ -263,6 +274,35 @@ class Sph:
         out = (C.c_uint64 * 2)()
         _check(_lib.sph_pair_stats(self._ctx, out))
         return int(out[0]), int(out[1])
+
+    def sph_balance_slabs(self, n_slabs: int):
+        """Planes (list of n_slabs + 1 cell-plane indices) that equalise the owned counts."""
+        out = (C.c_int32 * (int(n_slabs) + 1))()
+        _check(_lib.sph_balance_slabs(self._ctx, int(n_slabs), out))
+        return [int(x) for x in out]
+
+    def sph_download_resume(self):
+        """(vel_m1 (n,3), rho_m1 (n,), step_index): the Verlet n-1 state in id order."""
+        vel = np.empty((self.n, 3), dtype=np.float32)
+        rho = np.empty(self.n, dtype=np.float32)
+        k = C.c_uint64(0)
+        _check(_lib.sph_download_resume(self._ctx, vel.ctypes.data, rho.ctypes.data, C.byref(k)))
+        return vel, rho, int(k.value)
+
+    def sph_set_resume(self, vel_m1, rho_m1, step_index: int):
+        a, dev_a, k1 = _ptr(np.ascontiguousarray(vel_m1, dtype=np.float32) if isinstance(vel_m1, np.ndarray) else vel_m1)
+        b, dev_b, k2 = _ptr(np.ascontiguousarray(rho_m1, dtype=np.float32) if isinstance(rho_m1, np.ndarray) else rho_m1)
+        assert dev_a == dev_b
+        _check(_lib.sph_set_resume(self._ctx, a, b, int(step_index), int(dev_a)))
+
+    def sph_last_cuda_error(self) -> str:
+        return _lib.sph_last_cuda_error(self._ctx).decode()
+
+    def sph_fma_peak(self, variant: int = 0, iters: int = 4096) -> float:
+        """Measured FP32 TFLOP/s of a register-resident FMA chain (0 = FFMA, 1 = packed FFMA2)."""
+        out = C.c_double(0.0)
+        _check(_lib.sph_fma_peak(self._ctx, int(variant), int(iters), C.byref(out)))
+        return float(out.value)
 
     def sph_launch_count(self) -> int:
         out = C.c_uint64(0)

@@ -155,27 +155,53 @@ cudaError_t launch_slab_meta(sph_ctx *c)
     return cudaGetLastError();
 }
 
-// ---- edge labels for new planes without re-sorting ---------------------------------------------
-__global__ void retag_kernel(uint32_t n, uint32_t *__restrict__ keyword, SlabC sl, int nyz)
+// ---- edge and migration labels for new planes without re-sorting ----------------------------------
+// Re-planing (sph_build_halos with planes that differ from the ones the sort tagged with; the
+// load-balancing step of SURVEY 8(f) NEXT-4): owner, edge label (L240) and migration
+// label (L264) of every particle are recomputed from its cell and the NEW planes; the previous owner
+// is the one the sort recorded next to the pair (kv.y >> 28).  A particle whose owner changes only
+// because a plane moved is a migrant like any other (reading A15).  The migrant counts per tile and
+// per group that the compaction needs are rebuilt in the same pass (tile = GATHER_THREADS slots, as
+// in gather_kernel).
+__global__ void __launch_bounds__(GATHER_THREADS)
+retag_kernel(uint32_t n, uint32_t *__restrict__ keyword, const uint2 *__restrict__ kv, SlabC sl, int nyz,
+             int have_prev, uint32_t *__restrict__ mig_tile, uint32_t *__restrict__ mig_grp)
 {
-    uint32_t j = blockIdx.x * blockDim.x + threadIdx.x;
-    if (j >= n) return;
-    uint32_t w = keyword[j];
-    int cx = (int)((w & CELL_MASK) / (uint32_t)nyz);
-    int slab = 0;
+    const uint32_t j = blockIdx.x * blockDim.x + threadIdx.x;
+    bool migrant = false;
+    if (j < n) {
+        const uint32_t w = keyword[j];
+        const int cx = (int)((w & CELL_MASK) / (uint32_t)nyz);
+        int slab = 0;
 #pragma unroll
-    for (int k = 1; k < SPH_MAX_SLABS; ++k) slab += (k < sl.n_slabs && cx >= sl.planes[k]) ? 1 : 0;
-    uint32_t lab = 0;
-    if (slab > 0 && cx == sl.planes[slab]) lab = 1;
-    if (slab < sl.n_slabs - 1 && cx == sl.planes[slab + 1] - 1) lab = 2;
-    keyword[j] = (w & ~(3u << TAG_SHIFT)) | (lab << TAG_SHIFT);
+        for (int k = 1; k < SPH_MAX_SLABS; ++k) slab += (k < sl.n_slabs && cx >= sl.planes[k]) ? 1 : 0;
+        uint32_t lab = 0;
+        if (slab > 0 && cx == sl.planes[slab]) lab = 1;
+        if (slab < sl.n_slabs - 1 && cx == sl.planes[slab + 1] - 1) lab = 2;
+        uint32_t mig = 0;
+        if (have_prev) {
+            const int prev = (int)(kv[j].y >> 28);
+            mig = slab < prev ? 1u : (slab > prev ? 2u : 0u);
+        }
+        migrant = mig != 0;
+        keyword[j] = (w & CELL_MASK) | ((lab | (mig << 2)) << TAG_SHIFT);
+    }
+    const int cnt = __syncthreads_count(migrant);
+    if (threadIdx.x == 0) {
+        mig_tile[blockIdx.x] = (uint32_t)cnt;
+        if (cnt) atomicAdd(&mig_grp[blockIdx.x / MG_SUB], (uint32_t)cnt);
+    }
 }
 
-cudaError_t launch_retag(sph_ctx *c)
+// have_prev: the last sort had previous owners (else nothing migrates: first sort, reading A15)
+cudaError_t launch_retag(sph_ctx *c, bool have_prev)
 {
     uint32_t n = (uint32_t)c->n;
     if (n == 0) return cudaSuccess;
-    retag_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(n, c->keyword, c->tagged_slabs, c->grid.nyz);
+    cudaError_t e = cudaMemsetAsync(c->mig_grp, 0, sizeof(uint32_t) * ((size_t)mig_groups(n) + 1), c->stream);
+    if (e != cudaSuccess) return e;
+    retag_kernel<<<gather_tiles(n), GATHER_THREADS, 0, c->stream>>>(n, c->keyword, c->kv[c->kv_sorted], c->tagged_slabs,
+                                                                   c->grid.nyz, have_prev ? 1 : 0, c->mig_tile, c->mig_grp);
     c->n_launches++;
     return cudaGetLastError();
 }

@@ -150,9 +150,11 @@ cudaError_t launch_migrants(sph_ctx *c)
     uint32_t n = (uint32_t)c->n;
     if (n == 0) return cudaSuccess;
     const uint32_t tiles = gather_tiles(n), groups = mig_groups(n);
-    // a fresh copy of the group counts each time: the scan runs in place and halos may be
-    // rebuilt (new planes) without a new sort
-    cudaError_t e = cudaMemcpyAsync(c->mig_off, c->mig_grp, sizeof(uint32_t) * groups, cudaMemcpyDeviceToDevice,
+    // counts restart at every compaction (halos may be rebuilt without a new sort)
+    cudaError_t e = cudaMemsetAsync(c->mig_count, 0, sizeof(uint32_t) * 2 * SPH_MAX_SLABS, c->stream);
+    if (e != cudaSuccess) return e;
+    // a fresh copy of the group counts each time: the scan runs in place
+    e = cudaMemcpyAsync(c->mig_off, c->mig_grp, sizeof(uint32_t) * groups, cudaMemcpyDeviceToDevice,
                                     c->stream);
     if (e != cudaSuccess) return e;
     mig_scan_kernel<<<1, MG_SCAN_THREADS, 0, c->stream>>>(groups, c->mig_off, c->mig_total);
@@ -162,6 +164,53 @@ cudaError_t launch_migrants(sph_ctx *c)
     mig_compact_kernel<<<groups, GATHER_THREADS, 0, c->stream>>>(
         n, tiles, c->mig_off, c->mig_tile, c->keyword, c->kv[c->kv_sorted], c->idt[c->cur], c->tagged_slabs, c->grid.nyz,
         c->migrants, c->mig_count);
+    c->n_launches++;
+    return cudaGetLastError();
+}
+
+// ---- movable slab planes ("domain decomposition with load
+// balancing", L389) --------------------------------------------------------------------------------
+// C[p] = number of particles in cell planes < p = cell_begin[p * nyz] (the cell table already holds
+// it).  Plane s (s = 1..S-1, left to right) = the p in [planes[s-1] + 2, ncx - 2 (S - s)] that minimises
+// |C[p] S - s N|, the lowest such p on ties (every slab keeps at least two cell planes, reading A14).
+// C is non-decreasing, so the minimum sits at the crossing point: a few binary searches by one thread.
+__global__ void balance_kernel(const uint32_t *__restrict__ cell_begin, int ncx, int nyz, uint32_t n, int S,
+                               int32_t *__restrict__ planes_out)
+{
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    auto C = [&](int p) -> unsigned long long { return (unsigned long long)cell_begin[(size_t)p * (size_t)nyz]; };
+    auto first_ge = [&](int lo, int hi, unsigned long long v_times_S) -> int {   // first p in [lo, hi] with C[p] S >= v, else hi + 1
+        int a = lo, b = hi + 1;
+        while (a < b) {
+            const int m = (a + b) >> 1;
+            if (C(m) * (unsigned long long)S >= v_times_S) b = m; else a = m + 1;
+        }
+        return a;
+    };
+    planes_out[0] = 0;
+    planes_out[S] = ncx;
+    int prev = 0;
+    for (int s = 1; s < S; ++s) {
+        const int lo = prev + 2, hi = ncx - 2 * (S - s);
+        const unsigned long long T = (unsigned long long)s * (unsigned long long)n;
+        const int a = first_ge(lo, hi, T);
+        int best;
+        if (a == lo) {
+            best = lo;
+        } else {
+            const unsigned long long below = C(a - 1) * (unsigned long long)S;      // < T
+            const int q = first_ge(lo, a - 1, below);                                // lowest plane of that plateau
+            if (a > hi) best = q;
+            else best = (T - below <= C(a) * (unsigned long long)S - T) ? q : a;
+        }
+        planes_out[s] = best;
+        prev = best;
+    }
+}
+
+cudaError_t launch_balance(sph_ctx *c, int n_slabs, int32_t *d_planes)
+{
+    balance_kernel<<<1, 32, 0, c->stream>>>(c->cell_begin, c->grid.nc[0], c->grid.nyz, (uint32_t)c->n, n_slabs, d_planes);
     c->n_launches++;
     return cudaGetLastError();
 }

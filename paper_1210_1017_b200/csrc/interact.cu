@@ -513,12 +513,6 @@ template <int KERNEL, bool UNIFORM, bool GAMMA7, bool MU>
 static cudaError_t launch_staged(sph_ctx *c)
 {
     auto kern = interact_staged_kernel<KERNEL, UNIFORM, GAMMA7, MU>;
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(IaSmem) + SPH_IA_PAD);
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
     int zb = c->zblock;
     int nzb = (c->grid.nc[2] + zb - 1) / zb;
     const IaOverride &ov = c->ia_ov;               // per-slab execution works on a local particle set
@@ -531,350 +525,6 @@ static cudaError_t launch_staged(sph_ctx *c)
         ov.on ? ov.pos4 : c->pos4[c->cur], ov.on ? ov.velrho4 : c->velrho4[c->cur], ov.on ? ov.idt : c->idt[c->cur],
         ov.on ? ov.keyword : c->keyword, ov.on ? ov.cell_begin : c->cell_begin, ov.on ? ov.acc4 : c->acc4, c->mumax,
         c->grid, c->phys, zb, nzb, thr_h, zlim, cx_first);
-    c->n_launches++;
-    return cudaGetLastError();
-}
-
-// ---- tile variant of the staged kernel (SPH_OPT_INTERACT_VARIANT = 2) -----------------------------------
-// Same filter / drain machinery, but a CTA owns TI_B x TI_B neighbouring columns (zb cells each), so its
-// targets share (TI_B + 2)^2 candidate columns instead of 9 per column: 8 staged candidates per target
-// instead of 11, a neighbourhood only (zb + 2) cells tall (tighter fp16 pad), and - what it is for -
-// 76 KB of shared memory per CTA, i.e. 3 CTAs = 21 warps per SM instead of 16.
-#ifndef SPH_TI_QCAP
-#define SPH_TI_QCAP 10
-#endif
-constexpr int TI_B = 2;
-constexpr int TI_COL = (TI_B + 2) * (TI_B + 2);
-constexpr int TI_THREADS = 224;
-constexpr int TI_QCAP = SPH_TI_QCAP;
-constexpr int TI_CAP = 1744;          // 16 columns x 4 cells x 27 + slack, multiple of 16
-constexpr int TI_ZMAX = 8;            // max cells per z-block of a tile (keeps the cell-begin table small)
-constexpr int TI_NBLK = TI_CAP / IA_BLK;
-static_assert(TI_CAP % IA_BLK == 0 && TI_NBLK <= 256, "block index must fit 8 bits of a stack entry");
-
-struct TiSmem {
-    float4 rel[TI_CAP + 1];
-    float4 vr[TI_CAP + 1];
-    uint4 hp[TI_NBLK * 6];
-    uint32_t stack[TI_QCAP * TI_THREADS];
-    uint32_t cbt[TI_COL][TI_ZMAX + 3];
-    uint32_t col_vstart[TI_COL + 1];
-    uint32_t stage_lo[TI_COL], stage_hi[TI_COL];
-    int32_t stage_off[TI_COL];
-    uint32_t tbase[TI_B * TI_B], tcount[TI_B * TI_B], tstart[TI_B * TI_B + 1];   // target ranges of the own columns
-};
-
-int interact_tile_threads() { return TI_THREADS; }
-int interact_tile_columns() { return TI_B * TI_B; }
-int interact_tile_zmax() { return TI_ZMAX; }
-static_assert(sizeof(TiSmem) + 16 <= 76800, "three CTAs per SM");
-
-template <int KERNEL, bool UNIFORM, bool GAMMA7, bool MU>
-__global__ void __launch_bounds__(TI_THREADS, 3)
-interact_tile_kernel(const float4 *__restrict__ pos4, const float4 *__restrict__ velrho4,
-                       const uint32_t *__restrict__ idt, const uint32_t *__restrict__ keyword,
-                       const uint32_t *__restrict__ cell_begin, float4 *__restrict__ acc4, float *__restrict__ mu_out,
-                       GridC g, PhysC ph, int zb, int nzb, float thr_h /* filter threshold, units of h^2 */,
-                       float zlim /* |z| bound the threshold was derived for, units of h */)
-{
-    extern __shared__ __align__(16) unsigned char ia_raw[];
-    TiSmem &S = *reinterpret_cast<TiSmem *>(ia_raw);
-    __shared__ uint32_t s_wide;       // some staged particle or target lies outside the fp16 error model
-    const int tid = threadIdx.x;
-
-    // ---- which tile: TI_B x TI_B columns, zb cells
-    uint32_t b = blockIdx.x;
-    const int bz = b % nzb;
-    b /= nzb;
-    const int nby = (g.nc[1] + TI_B - 1) / TI_B;
-    const int cy0 = (int)(b % nby) * TI_B;
-    const int cx0 = (int)(b / nby) * TI_B;
-    const int cz0 = bz * zb, cz1 = min(cz0 + zb, g.nc[2]);
-    const int zlo = max(cz0 - 1, 0), zhi = min(cz1 + 1, g.nc[2]);
-    const int nz = zhi - zlo;                                    // <= zb + 2
-    // ---- empty tiles (most of a dam-break tank) leave at once: every thread reads the four ranges
-    {
-        uint32_t any = 0;
-#pragma unroll
-        for (int t = 0; t < TI_B * TI_B; ++t) {
-            const int x = cx0 + t / TI_B, y = cy0 + t % TI_B;
-            if (x < g.nc[0] && y < g.nc[1]) {
-                const uint32_t colbase = (uint32_t)(x * g.nc[1] + y) * g.nc[2];
-                any |= cell_begin[colbase + cz1] - cell_begin[colbase + cz0];
-            }
-        }
-        if (any == 0) return;
-    }
-    if (tid == 0) {
-        s_wide = 0u;
-        S.rel[TI_CAP] = make_float4(IA_FAR, IA_FAR, IA_FAR, 0.f);
-        S.vr[TI_CAP] = make_float4(0.f, 0.f, 0.f, 1.f);
-    }
-    // ---- target ranges of the TI_B x TI_B own columns, concatenated
-    if (tid < TI_B * TI_B) {
-        const int x = cx0 + tid / TI_B, y = cy0 + tid % TI_B;
-        uint32_t tb = 0, te = 0;
-        if (x < g.nc[0] && y < g.nc[1]) {
-            const uint32_t colbase = (uint32_t)(x * g.nc[1] + y) * g.nc[2];
-            tb = cell_begin[colbase + cz0];
-            te = cell_begin[colbase + cz1];
-        }
-        S.tbase[tid] = tb;
-        S.tcount[tid] = te - tb;
-    }
-    // ---- cell-begin table of the (TI_B + 2)^2 candidate columns
-    for (int k = tid; k < TI_COL * (nz + 1); k += TI_THREADS) {
-        int col = k / (nz + 1), z = k % (nz + 1);
-        int x = cx0 + col / (TI_B + 2) - 1, y = cy0 + col % (TI_B + 2) - 1;
-        uint32_t v = 0;
-        if (x >= 0 && x < g.nc[0] && y >= 0 && y < g.nc[1])
-            v = cell_begin[(uint32_t)(x * g.nc[1] + y) * g.nc[2] + zlo + z];
-        S.cbt[col][z] = v;          // columns outside the grid: all 0 => empty ranges
-    }
-    // ---- CTA-relative coordinate origin (same value in every thread)
-    const float cell = 2.0f * ph.h;
-    const float ox = rel_origin(fmaf((float)cx0, cell, g.min[0]), (float)(TI_B + 3) * cell);
-    const float oy = rel_origin(fmaf((float)cy0, cell, g.min[1]), (float)(TI_B + 3) * cell);
-    const float oz = rel_origin(fmaf((float)cz0, cell, g.min[2]), (float)(zb + 3) * cell);
-    // centre of the neighbourhood in that frame, and the scale of the fp16 filter copy (units of h):
-    // |x|, |y| <= TI_B + 2 and |z| <= nz for every particle that lies inside its cell
-    const float inv_h = 2.0f * ph.inv_h_half;
-    const float ccx = fmaf((float)cx0 + 0.5f * (float)TI_B, cell, g.min[0]) - ox;
-    const float ccy = fmaf((float)cy0 + 0.5f * (float)TI_B, cell, g.min[1]) - oy;
-    const float ccz = fmaf((float)zlo + 0.5f * (float)nz, cell, g.min[2]) - oz;
-    __syncthreads();
-    if (tid == 0) {
-        uint32_t acc = 0;
-        for (int col = 0; col < TI_COL; ++col) {
-            S.col_vstart[col] = acc;
-            acc += S.cbt[col][nz] - S.cbt[col][0];
-        }
-        S.col_vstart[TI_COL] = acc;
-        acc = 0;
-        for (int t = 0; t < TI_B * TI_B; ++t) { S.tstart[t] = acc; acc += S.tcount[t]; }
-        S.tstart[TI_B * TI_B] = acc;
-    }
-    __syncthreads();
-    const uint32_t total = S.col_vstart[TI_COL];
-    const uint32_t ttotal = S.tstart[TI_B * TI_B];
-    if (ttotal == 0) return;                                     // CTA-uniform
-    const uint32_t lane_full = 0xffffffffu;
-    const uint32_t rel_base = (uint32_t)__cvta_generic_to_shared(S.rel);
-    const uint32_t vr_delta = (uint32_t)__cvta_generic_to_shared(S.vr) - rel_base;
-    const uint32_t hp_base = (uint32_t)__cvta_generic_to_shared(S.hp);
-    const uint32_t stk_base = (uint32_t)__cvta_generic_to_shared(S.stack) + 4u * tid;
-    constexpr uint32_t STK_STRIDE = 4u * TI_THREADS;
-    const uint32_t stk_high = stk_base + STK_STRIDE * (TI_QCAP - 1);   // sp above this = stack full
-
-    for (uint32_t chunk = 0; chunk < ttotal; chunk += TI_THREADS) {
-        const uint32_t q = chunk + tid;
-        const bool active = q < ttotal;
-        int tcol = 0;
-#pragma unroll
-        for (int t = 1; t < TI_B * TI_B; ++t) tcol += (active && q >= S.tstart[t]) ? 1 : 0;
-        const uint32_t i = active ? S.tbase[tcol] + (q - S.tstart[tcol]) : 0u;
-        const int tx = tcol / TI_B, ty = tcol % TI_B;
-        const uint32_t own_col = (uint32_t)((cx0 + tx) * g.nc[1] + (cy0 + ty)) * g.nc[2];
-        float4 pi = make_float4(ox + ccx, oy + ccy, oz + ccz, 0.f), vi = make_float4(0.f, 0.f, 0.f, 1.f);
-        int kz = 0;
-        bool fluid = false;
-        if (active) {
-            pi = pos4[i];
-            vi = velrho4[i];
-            fluid = (idt[i] & TYPE_BIT) == 0;
-            kz = (int)((keyword[i] & CELL_MASK) - own_col) - zlo;   // own cz - zlo
-        }
-        const float xi = pi.x - ox, yi = pi.y - oy, zi = pi.z - oz;  // exact
-        // fp16 filter copy of the target; a target outside the error model widens the CTA's filter
-        const float xs = (xi - ccx) * inv_h, ys = (yi - ccy) * inv_h, zs = (zi - ccz) * inv_h;
-        if (!(fabsf(xs) < 8.0f && fabsf(ys) < 8.0f && fabsf(zs) < zlim)) s_wide = 1u;
-        const __half2 hxi = __float2half2_rn(xs), hyi = __float2half2_rn(ys), hzi = __float2half2_rn(zs);
-        const float ci = sound_speed<GAMMA7>(vi.w, ph);
-        const int k_lo = max(kz - 1, 0), k_hi = min(kz + 2, nz);   // own 3-cell window in cbt rows
-        float ax = 0.f, ay = 0.f, az = 0.f, dr = 0.f, mumax = 0.f;
-        uint32_t sp = stk_base;                                     // shared address of the stack top
-        uint32_t cur_mask = 0, cur_s = 0;                           // entry being drained
-
-        // next pending candidate of this lane: smem index s, or ok = false
-        auto pop = [&](uint32_t &s, bool &ok) {
-            if (cur_mask == 0 && sp > stk_base) {
-                sp -= STK_STRIDE;
-                const uint32_t e = lds_u32(sp);
-                cur_mask = e & 0xFFFFu;                              // bit c = candidate c of the block
-                cur_s = (e >> 12) & 0xFF0u;                          // block index * 16
-            }
-            ok = cur_mask != 0;
-            s = cur_s + (uint32_t)(__ffs(cur_mask) - 1);            // garbage if !ok
-            cur_mask &= cur_mask - 1;
-        };
-        // pair term of candidate s; ok = false turns it into a no-op without a branch: the partner is
-        // the far-away dummy slot, whose F is 0.  The exact fp32 distance is
-        // formed here: a candidate the fp16 filter let through although it lies outside 2h adds
-        // exactly 0 because F is clamped.
-        auto interact = [&](uint32_t s, bool ok) {
-            s = ok ? s : (uint32_t)TI_CAP;
-            const float4 rj = lds_f4(rel_base + 16u * s);
-            float4 vj = lds_f4(rel_base + vr_delta + 16u * s);
-            const float dx = xi - rj.x, dy = yi - rj.y, dz = zi - rj.z;     // == absolute differences
-            const float r2 = fmaxf(fmaf(dz, dz, fmaf(dy, dy, dx * dx)), IA_TINY);
-            float mj = 1.0f;
-            if (!UNIFORM) {
-                mj = vj.w < 0.f ? ph.mass_bound : ph.mass_fluid;
-                vj.w = fabsf(vj.w);
-            }
-            pair_term<KERNEL, GAMMA7, MU>(dx, dy, dz, r2, vi.x, vi.y, vi.z, vi.w, pi.w, ci, vj, rj.w, mj, ph,
-                                          ax, ay, az, dr, mumax);
-        };
-        // one drain round: up to IA_DRAIN pending pairs per lane, as interleaved dependency chains
-        auto drain_round = [&]() {
-            uint32_t s[IA_DRAIN];
-            bool ok[IA_DRAIN];
-#pragma unroll
-            for (int q = 0; q < IA_DRAIN; ++q) pop(s[q], ok[q]);
-#pragma unroll
-            for (int q = 0; q < IA_DRAIN; ++q) interact(s[q], ok[q]);
-        };
-
-        for (uint32_t bstart = 0; bstart < total; bstart += TI_CAP) {
-            const uint32_t bend = min(total, bstart + TI_CAP);
-            __syncthreads();                       // previous batch / chunk fully consumed
-            if (tid < TI_COL) {
-                uint32_t vs = S.col_vstart[tid], ve = S.col_vstart[tid + 1];
-                uint32_t lo = max(vs, bstart), hi = min(ve, bend);
-                uint32_t gb = S.cbt[tid][0];
-                if (lo < hi) {
-                    S.stage_lo[tid] = gb + (lo - vs);
-                    S.stage_hi[tid] = gb + (hi - vs);
-                    S.stage_off[tid] = (int32_t)(lo - bstart) - (int32_t)(gb + (lo - vs));
-                } else {
-                    S.stage_lo[tid] = 0; S.stage_hi[tid] = 0; S.stage_off[tid] = 0;
-                }
-            }
-            __syncthreads();
-            // ---- stage: the batch is the virtual concatenation [bstart, bend) of the 9 column ranges and
-            // smem index = virtual index - bstart.  Four candidates per thread per round with all their
-            // global loads issued before the first use, so a round costs one memory latency, not four.
-            const uint32_t nst = bend - bstart;
-            for (uint32_t k0 = tid; k0 < nst; k0 += 4u * TI_THREADS) {
-                float4 p[4], v[4];
-                bool bnd[4];
-#pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    const uint32_t si = k0 + (uint32_t)u * TI_THREADS;
-                    bnd[u] = false;
-                    if (si < nst) {
-                        const uint32_t vv = bstart + si;
-                        int col = 0;
-#pragma unroll
-                        for (int q = 1; q < TI_COL; ++q) col += (vv >= S.col_vstart[q]) ? 1 : 0;
-                        const uint32_t j = S.cbt[col][0] + (vv - S.col_vstart[col]);
-                        p[u] = __ldg(pos4 + j);
-                        v[u] = __ldg(velrho4 + j);
-                        if (!UNIFORM) bnd[u] = (__ldg(idt + j) & TYPE_BIT) != 0;
-                    }
-                }
-#pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    const uint32_t si = k0 + (uint32_t)u * TI_THREADS;
-                    if (si < nst) {
-                        if (!UNIFORM && bnd[u]) v[u].w = -v[u].w;
-                        const float xr = p[u].x - ox, yr = p[u].y - oy, zr = p[u].z - oz;
-                        S.rel[si] = make_float4(xr, yr, zr, p[u].w);
-                        S.vr[si] = v[u];
-                        const float xq = (xr - ccx) * inv_h, yq = (yr - ccy) * inv_h, zq = (zr - ccz) * inv_h;
-                        if (!(fabsf(xq) < 8.0f && fabsf(yq) < 8.0f && fabsf(zq) < zlim)) s_wide = 1u;
-                        // block si / 16: x words at +0, y at +32, z at +64; candidate c = si % 16 is half c / 8 of word c % 8
-                        const uint32_t a = hp_base + 96u * (si >> 4) + 4u * (si & 7u) + ((si >> 2) & 2u);
-                        sts_u16(a, __half_as_ushort(__float2half_rn(xq)));
-                        sts_u16(a + 32u, __half_as_ushort(__float2half_rn(yq)));
-                        sts_u16(a + 64u, __half_as_ushort(__float2half_rn(zq)));
-                    }
-                }
-            }
-            __syncthreads();
-            // a particle outside the fp16 error model (it left the grid and sits clamped in an edge
-            // cell): let every candidate through, the drain decides exactly
-            const __half2 thr = __float2half2_rn(s_wide ? 65504.0f : thr_h);
-
-            const bool wide = s_wide != 0u;
-
-            // ---- filter + drain.  Blocks of 16 candidates are aligned in shared memory; the first
-            // and the last block of a lane's range are trimmed with masks in the entry's bit layout.
-            for (int w9 = 0; w9 < 9; ++w9) {
-                const int col = (tx + w9 / 3) * (TI_B + 2) + ty + w9 % 3;      // per lane
-                int lo = 0, hi = 0;
-                if (active) {
-                    lo = (int)max(S.cbt[col][k_lo], S.stage_lo[col]);
-                    hi = (int)min(S.cbt[col][k_hi], S.stage_hi[col]);
-                }
-                const int off = S.stage_off[col];
-                const bool work = hi > lo;
-                const uint32_t slo = work ? (uint32_t)(lo + off) : 0u, shi = work ? (uint32_t)(hi + off) : 0u;
-                const uint32_t blk_lo = slo >> 4;
-                const int nblk = work ? (int)(((shi + 15u) >> 4) - blk_lo) : 0;
-                const int maxblk = __reduce_max_sync(lane_full, nblk);
-                uint32_t lin = (0xFFFFu << (slo & 15u)) & 0xFFFFu;                    // candidates >= slo
-                const uint32_t first_mask = (lin & 0xFFu) | ((lin & 0xFF00u) << 8);
-                lin = 0xFFFFu >> ((16u - (shi & 15u)) & 15u);                          // candidates < shi
-                const uint32_t last_mask = (lin & 0xFFu) | ((lin & 0xFF00u) << 8);
-                for (int it = 0; it < maxblk; ++it) {
-                    const uint32_t blk = min(blk_lo + (uint32_t)it, (uint32_t)(TI_NBLK - 1));
-                    const uint32_t a0 = hp_base + 96u * blk;
-                    const uint4 x0 = lds_u4(a0), x1 = lds_u4(a0 + 16u);
-                    const uint4 y0 = lds_u4(a0 + 32u), y1 = lds_u4(a0 + 48u);
-                    const uint4 z0 = lds_u4(a0 + 64u), z1 = lds_u4(a0 + 80u);
-                    uint32_t m;
-                    m = filt2h(hxi, hyi, hzi, x0.x, y0.x, z0.x, thr) & 0x00010001u;
-                    m |= filt2h(hxi, hyi, hzi, x0.y, y0.y, z0.y, thr) & 0x00020002u;
-                    m |= filt2h(hxi, hyi, hzi, x0.z, y0.z, z0.z, thr) & 0x00040004u;
-                    m |= filt2h(hxi, hyi, hzi, x0.w, y0.w, z0.w, thr) & 0x00080008u;
-                    m |= filt2h(hxi, hyi, hzi, x1.x, y1.x, z1.x, thr) & 0x00100010u;
-                    m |= filt2h(hxi, hyi, hzi, x1.y, y1.y, z1.y, thr) & 0x00200020u;
-                    m |= filt2h(hxi, hyi, hzi, x1.z, y1.z, z1.z, thr) & 0x00400040u;
-                    m |= filt2h(hxi, hyi, hzi, x1.w, y1.w, z1.w, thr) & 0x00800080u;
-                    if (wide) m = 0x00FF00FFu;
-                    if (it == 0) m &= first_mask;
-                    if (it == nblk - 1) m &= last_mask;
-                    if (it < nblk && m) {                   // entry: linear 16-bit mask | block index << 16
-                        sts_u32(sp, (m & 0xFFu) | ((m >> 8) & 0xFF00u) | (blk << 16));
-                        sp += STK_STRIDE;
-                    }
-                    while (__any_sync(lane_full, sp > stk_high)) drain_round();
-                }
-            }
-            // ---- flush the stacks before the staged data is replaced.  Until here the stacks are
-            // kept as full as they can be (drains only when some lane's stack is full), so that
-            // nearly every lane has a pending pair in every drain round.
-            while (__any_sync(lane_full, (sp > stk_base) || cur_mask != 0)) drain_round();
-        }
-        if (active) {
-            if (UNIFORM) { ax *= ph.mass_fluid; ay *= ph.mass_fluid; az *= ph.mass_fluid; dr *= ph.mass_fluid; }
-            if (fluid) { ax += ph.g[0]; ay += ph.g[1]; az += ph.g[2]; }
-            else { ax = ay = az = 0.f; }
-            acc4[i] = make_float4(ax, ay, az, dr);
-            if (MU) mu_out[i] = mumax;
-        }
-    }
-}
-
-template <int KERNEL, bool UNIFORM, bool GAMMA7, bool MU>
-static cudaError_t launch_tile(sph_ctx *c)
-{
-    auto kern = interact_tile_kernel<KERNEL, UNIFORM, GAMMA7, MU>;
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(TiSmem));
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
-    int zb = c->zblock_tile;
-    int nzb = (c->grid.nc[2] + zb - 1) / zb;
-    uint64_t blocks = (uint64_t)((c->grid.nc[0] + TI_B - 1) / TI_B) * ((c->grid.nc[1] + TI_B - 1) / TI_B) * nzb;
-    float thr_h, zlim;
-    filter_threshold(zb, &thr_h, &zlim);
-    kern<<<(uint32_t)blocks, TI_THREADS, sizeof(TiSmem), c->stream>>>(
-        c->pos4[c->cur], c->velrho4[c->cur], c->idt[c->cur], c->keyword, c->cell_begin, c->acc4, c->mumax,
-        c->grid, c->phys, zb, nzb, thr_h, zlim);
     c->n_launches++;
     return cudaGetLastError();
 }
@@ -943,20 +593,34 @@ static cudaError_t launch_interact_mu(sph_ctx *c)
         if (k == 0) return g7 ? launch_simple<0, true, MU>(c) : launch_simple<0, false, MU>(c);
         return g7 ? launch_simple<1, true, MU>(c) : launch_simple<1, false, MU>(c);
     }
-    if (c->interact_variant == 2) {
-        if (k == 0) {
-            if (uni) return g7 ? launch_tile<0, true, true, MU>(c) : launch_tile<0, true, false, MU>(c);
-            return g7 ? launch_tile<0, false, true, MU>(c) : launch_tile<0, false, false, MU>(c);
-        }
-        if (uni) return g7 ? launch_tile<1, true, true, MU>(c) : launch_tile<1, true, false, MU>(c);
-        return g7 ? launch_tile<1, false, true, MU>(c) : launch_tile<1, false, false, MU>(c);
-    }
     if (k == 0) {
         if (uni) return g7 ? launch_staged<0, true, true, MU>(c) : launch_staged<0, true, false, MU>(c);
         return g7 ? launch_staged<0, false, true, MU>(c) : launch_staged<0, false, false, MU>(c);
     }
     if (uni) return g7 ? launch_staged<1, true, true, MU>(c) : launch_staged<1, true, false, MU>(c);
     return g7 ? launch_staged<1, false, true, MU>(c) : launch_staged<1, false, false, MU>(c);
+}
+
+// Dynamic shared memory opt-in of every instance of the staged kernel, for the CURRENT device (the
+// attribute is per device; sph_init calls this for every new context).
+template <int KERNEL, bool UNIFORM, bool GAMMA7>
+static cudaError_t configure_staged()
+{
+    cudaError_t e = cudaFuncSetAttribute(interact_staged_kernel<KERNEL, UNIFORM, GAMMA7, false>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(IaSmem) + SPH_IA_PAD);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(interact_staged_kernel<KERNEL, UNIFORM, GAMMA7, true>,
+                                cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(IaSmem) + SPH_IA_PAD);
+}
+
+cudaError_t configure_interact()
+{
+    cudaError_t e = cudaSuccess;
+#define SPH_CFG(K, U, G) if (e == cudaSuccess) e = configure_staged<K, U, G>()
+    SPH_CFG(0, true, true); SPH_CFG(0, true, false); SPH_CFG(0, false, true); SPH_CFG(0, false, false);
+    SPH_CFG(1, true, true); SPH_CFG(1, true, false); SPH_CFG(1, false, true); SPH_CFG(1, false, false);
+#undef SPH_CFG
+    return e;
 }
 
 // with_mu: also write max_j |mu_ij| per particle (needed by the variable time step only)

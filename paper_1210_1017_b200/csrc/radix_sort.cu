@@ -232,18 +232,17 @@ onesweep_kernel(uint32_t n, const uint2 *__restrict__ in, uint2 *__restrict__ ou
     else onesweep_tile<false>(S, n, in, out, hist, tile_state, shift, dmask, tile);
 }
 
+// per-device attribute, set by sph_init for every new context
+cudaError_t configure_sort()
+{
+    return cudaFuncSetAttribute(onesweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(RsSmem));
+}
+
 cudaError_t launch_sort(sph_ctx *c)
 {
     uint32_t n = (uint32_t)c->n;
     c->kv_sorted = c->passes & 1;
     if (n == 0) return cudaSuccess;
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(onesweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)sizeof(RsSmem));
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
     uint32_t tiles = c->rs_tiles;
     cudaError_t e = cudaMemsetAsync(c->tile_state, 0, sizeof(uint32_t) * 256 * (size_t)tiles * c->passes, c->stream);
     if (e != cudaSuccess) return e;

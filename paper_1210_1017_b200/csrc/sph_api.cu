@@ -86,11 +86,19 @@ bool make_layout(const sph_params *p, uint64_t n, int max_slabs, Layout *L)
     return true;
 }
 
+// The library never prints: the text of the last failed CUDA call is kept for sph_last_cuda_error
+// (per context, and in a per-thread slot for failures before a context exists).
+thread_local char g_last_cuda_error[160] = "";
+
 int cuda_fail(sph_ctx *c, cudaError_t e)
 {
     if (e == cudaSuccess) return SPH_OK;
-    if (c) c->sticky = SPH_ERR_CUDA;
-    fprintf(stderr, "libsph_b200: CUDA error: %s\n", cudaGetErrorString(e));
+    const char *msg = cudaGetErrorString(e);
+    snprintf(g_last_cuda_error, sizeof(g_last_cuda_error), "%s", msg ? msg : "unknown CUDA error");
+    if (c) {
+        c->sticky = SPH_ERR_CUDA;
+        snprintf(c->last_cuda_error, sizeof(c->last_cuda_error), "%s", g_last_cuda_error);
+    }
     return SPH_ERR_CUDA;
 }
 #define CK(c, call)                                       \
@@ -202,6 +210,8 @@ int upload_state(sph_ctx *c, const sph_particles *part)
     CK(c, launch_init_state(c, dpos, dvel, drho, dtype));
     if (!part->on_device) CK(c, cudaStreamSynchronize(c->stream));   // host arrays may be reused
     c->have_prev_ranges = false;
+    c->sort_had_prev = false;
+    c->id_order = true;
     c->sorted_valid = c->halos_valid = c->rates_valid = c->mu_valid = false;
     c->step_index = 0;
     return SPH_OK;
@@ -303,12 +313,14 @@ int sph_init(sph_ctx **out, const sph_params *p, const sph_particles *part, int 
     if (zb < 1) zb = 1;
     if (zb > 32) zb = 32;
     c->zblock = zb;
-    int zt = (int)floor((double)interact_tile_threads() * 0.97 / ((ppc > 0.05 ? ppc : 0.05) * interact_tile_columns()));
-    if (zt < 1) zt = 1;
-    if (zt > interact_tile_zmax()) zt = interact_tile_zmax();
-    c->zblock_tile = zt;
 
-    cudaError_t e = cudaMemsetAsync(c->acc4, 0, 16 * (c->n ? c->n : 1), c->stream);
+    c->last_cuda_error[0] = 0;
+    c->id_order = true;
+    c->sort_had_prev = false;
+    // kernel attributes are per device: set them for the device this context lives on
+    cudaError_t e = configure_interact();
+    if (e == cudaSuccess) e = configure_sort();
+    if (e == cudaSuccess) e = cudaMemsetAsync(c->acc4, 0, 16 * (c->n ? c->n : 1), c->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->mig_total, 0, 4, c->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->mig_count, 0, 4 * 2 * SPH_MAX_SLABS, c->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->halo_offset, 0, 4 * (2 * SPH_MAX_SLABS + 1), c->stream);
@@ -357,6 +369,7 @@ int sph_sort_and_cells(sph_ctx *c)
 {
     if (!c) return SPH_ERR_ARG;
     if (c->sticky) return c->sticky;
+    c->sort_had_prev = c->have_prev_init || c->have_prev_ranges;
     {
         Timed t(c, SPH_T_KEYS);
         CK(c, launch_keys(c));
@@ -377,6 +390,7 @@ int sph_sort_and_cells(sph_ctx *c)
     }
     c->have_prev_init = false;
     c->have_prev_ranges = true;
+    c->id_order = false;
     c->sorted_valid = true;
     c->halos_valid = false;
     c->rates_valid = false;
@@ -396,10 +410,11 @@ int sph_build_halos(sph_ctx *c, const int32_t *planes, int n_slabs)
     {
         Timed t(c, SPH_T_HALO);
         if (!same_slabs(c->slabs, c->tagged_slabs)) {
+            // new planes without a new sort: owners, edge and migration labels, slab and halo ranges
             c->tagged_slabs = c->slabs;
-            CK(c, launch_retag(c));
-        }
-        CK(c, launch_slab_meta(c));
+            CK(c, launch_retag(c, c->sort_had_prev));
+            CK(c, launch_slab_meta(c));
+        }                                   // else: the ranges the sort left are current
         CK(c, launch_halo_gather(c));
     }
     {
@@ -458,7 +473,7 @@ int sph_interact_slab(sph_ctx *c, int slab)
     if (!c->sorted_valid || !c->halos_valid) return SPH_ERR_ORDER;
     const int S = c->tagged_slabs.n_slabs;
     if (slab < 0 || slab >= S) return SPH_ERR_ARG;
-    if (c->max_slabs < 2 && S > 1) return SPH_ERR_ARG;
+    if (c->max_slabs < 2) return SPH_ERR_ARG;     // the local cell table exists only for max_slabs >= 2
     uint32_t h_begin[SPH_MAX_SLABS + 1], h_range[4 * SPH_MAX_SLABS], h_off[2 * SPH_MAX_SLABS + 1];
     memset(h_range, 0, sizeof(h_range));
     memset(h_off, 0, sizeof(h_off));
@@ -640,6 +655,83 @@ int sph_pair_stats(sph_ctx *c, uint64_t *out)
     out[0] = h[0];
     out[1] = h[1];
     return SPH_OK;
+}
+
+int sph_download_resume(sph_ctx *c, float *vel_m1, float *rho_m1, uint64_t *step_index)
+{
+    if (!c) return SPH_ERR_ARG;
+    if (c->sticky) return c->sticky;
+    const uint64_t n = c->n;
+    if (step_index) *step_index = c->step_index;
+    if (n == 0 || (!vel_m1 && !rho_m1)) return SPH_OK;
+    int o = 1 - c->cur;                                   // idle halves as packed id-order staging
+    float *svel = (float *)c->velrho4[o], *srho = (float *)c->idt[o];
+    CK(c, launch_m1_pack(c, vel_m1 ? svel : nullptr, rho_m1 ? srho : nullptr));
+    if (vel_m1) CK(c, cudaMemcpyAsync(vel_m1, svel, 12 * n, cudaMemcpyDeviceToHost, c->stream));
+    if (rho_m1) CK(c, cudaMemcpyAsync(rho_m1, srho, 4 * n, cudaMemcpyDeviceToHost, c->stream));
+    CK(c, cudaStreamSynchronize(c->stream));
+    return SPH_OK;
+}
+
+int sph_set_resume(sph_ctx *c, const float *vel_m1, const float *rho_m1, uint64_t step_index, int on_device)
+{
+    if (!c || !vel_m1 || !rho_m1) return SPH_ERR_ARG;
+    if (c->sticky) return c->sticky;
+    if (!c->id_order) return SPH_ERR_ORDER;               // only right after sph_init / sph_set_state
+    const uint64_t n = c->n;
+    const float *dvel = vel_m1, *drho = rho_m1;
+    if (n && !on_device) {
+        float *svel = (float *)c->velrho4[1 - c->cur], *srho = (float *)c->idt[1 - c->cur];
+        CK(c, cudaMemcpyAsync(svel, vel_m1, 12 * n, cudaMemcpyHostToDevice, c->stream));
+        CK(c, cudaMemcpyAsync(srho, rho_m1, 4 * n, cudaMemcpyHostToDevice, c->stream));
+        dvel = svel; drho = srho;
+    }
+    CK(c, launch_m1_unpack(c, dvel, drho));
+    if (!on_device) CK(c, cudaStreamSynchronize(c->stream));
+    c->step_index = step_index;
+    return SPH_OK;
+}
+
+int sph_balance_slabs(sph_ctx *c, int n_slabs, int32_t *planes_out)
+{
+    if (!c || !planes_out || n_slabs < 1 || n_slabs > c->max_slabs) return SPH_ERR_ARG;
+    if (c->sticky) return c->sticky;
+    if (!c->sorted_valid) return SPH_ERR_ORDER;
+    if (c->grid.nc[0] < 2 * n_slabs && n_slabs > 1) return SPH_ERR_SLABS;
+    int32_t *d_planes = (int32_t *)c->dt_red;             // 32 words of scratch, dead outside sph_time_step
+    CK(c, launch_balance(c, n_slabs, d_planes));
+    CK(c, cudaMemcpyAsync(planes_out, d_planes, 4 * (n_slabs + 1), cudaMemcpyDeviceToHost, c->stream));
+    CK(c, cudaStreamSynchronize(c->stream));
+    return planes_ok(planes_out, n_slabs, c->grid.nc[0], c->max_slabs) ? SPH_OK : SPH_ERR_SLABS;
+}
+
+int sph_fma_peak(sph_ctx *c, int variant, int iters, double *tflops)
+{
+    if (!c || !tflops || iters < 1 || (variant != 0 && variant != 1)) return SPH_ERR_ARG;
+    if (c->sticky) return c->sticky;
+    const int blocks = NUM_SMS * 8;
+    cudaEvent_t e0, e1;
+    CK(c, cudaEventCreate(&e0));
+    CK(c, cudaEventCreate(&e1));
+    float *sink = (float *)c->scratch64;
+    int rc = SPH_OK;
+    cudaError_t e = launch_fma_peak(c, variant, iters / 8 + 1, blocks, sink);      // warm-up
+    if (e == cudaSuccess) e = cudaEventRecord(e0, c->stream);
+    if (e == cudaSuccess) e = launch_fma_peak(c, variant, iters, blocks, sink);
+    if (e == cudaSuccess) e = cudaEventRecord(e1, c->stream);
+    if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+    float ms = 0.f;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+    if (e != cudaSuccess) rc = cuda_fail(c, e);
+    else *tflops = 2.0 * 8.0 * 8.0 * (double)iters * 256.0 * (double)blocks / ((double)ms * 1e-3) / 1e12;
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    return rc;
+}
+
+const char *sph_last_cuda_error(const sph_ctx *c)
+{
+    return c ? c->last_cuda_error : g_last_cuda_error;
 }
 
 int sph_launch_count(const sph_ctx *c, uint64_t *out)

@@ -115,6 +115,7 @@ struct sph_ctx {
 
     bool have_prev_init;       // prev_init valid for the next sort
     bool have_prev_ranges;     // slab_begin valid as previous-owner ranges
+    bool sort_had_prev;        // the last sort labelled migrants (it had previous owners)
     bool sorted_valid;         // arrays sorted + cell table valid for the current positions
     bool halos_valid;
     bool rates_valid;
@@ -123,9 +124,10 @@ struct sph_ctx {
     uint64_t step_index;
     int interact_variant;
     int zblock;                // cells per z-block of the staged interaction kernel
-    int zblock_tile;           // same for the tile variant
 
     uint64_t n_launches;       // kernels launched so far (memsets and copies not counted)
+    bool id_order;             // live state arrays are still in id order (no sort since the last upload)
+    char last_cuda_error[160]; // text of the last failed CUDA call (sph_last_cuda_error)
 
     sph::StageTimer timer;
     sph::IaOverride ia_ov;     // off except inside sph_interact_slab
@@ -142,7 +144,7 @@ cudaError_t launch_sort(sph_ctx *c);
 cudaError_t launch_gather_cells(sph_ctx *c);
 cudaError_t launch_cell_fill(sph_ctx *c);
 cudaError_t launch_slab_meta(sph_ctx *c);
-cudaError_t launch_retag(sph_ctx *c);
+cudaError_t launch_retag(sph_ctx *c, bool have_prev);
 cudaError_t launch_halo_gather(sph_ctx *c);
 cudaError_t launch_migrants(sph_ctx *c);
 cudaError_t launch_interact(sph_ctx *c, bool with_mu);
@@ -154,15 +156,19 @@ cudaError_t launch_verlet(sph_ctx *c, float dt, int corrective);
 cudaError_t launch_pair_stats(sph_ctx *c, unsigned long long *d_out);
 cudaError_t launch_download_pack(sph_ctx *c, float *pos3, float *vel3, float *rho, float *acc3,
                                  float *drho);
+cudaError_t launch_m1_pack(sph_ctx *c, float *vel3, float *rho);
+cudaError_t launch_m1_unpack(sph_ctx *c, const float *vel3, const float *rho);
+cudaError_t launch_balance(sph_ctx *c, int n_slabs, int32_t *d_planes);
+cudaError_t launch_fma_peak(sph_ctx *c, int variant, int iters, int blocks, float *sink);
+// per-device kernel attributes (dynamic shared memory opt-in), set for every new context
+cudaError_t configure_interact();
+cudaError_t configure_sort();
 
 uint32_t radix_tiles(uint64_t n);
 uint32_t gather_tiles(uint64_t n);
 uint32_t mig_groups(uint64_t n);
 size_t gap_list_entries(uint64_t ncells);
 int interact_threads();
-int interact_tile_threads();
-int interact_tile_columns();
-int interact_tile_zmax();
 
 // Tait pressure over rho^2 from rho, fp32, cancellation-free.
 __device__ __forceinline__ float tait_p_over_rho2(float rho, const PhysC &ph)

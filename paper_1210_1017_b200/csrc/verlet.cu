@@ -36,7 +36,10 @@ verlet_kernel(uint32_t n, float4 *__restrict__ pos4, float4 *__restrict__ velrho
         p.z = fmaf(hdt2, a.z, fmaf(dt, v.z, p.z));
     }
     vn.w = rho_new;
-    if (!(isfinite(p.x) && isfinite(p.y) && isfinite(p.z) && isfinite(rho_new) && rho_new > 0.f))
+    // one test covers position, velocity, density and the rates they came from (inf - inf and 0 * inf
+    // are NaN, so the sum is finite exactly when every term is)
+    const float chk = (p.x + p.y + p.z) + (vn.x + vn.y + vn.z) + rho_new + (a.x + a.y + a.z + a.w);
+    if (!(isfinite(chk) && rho_new > 0.f))
         atomicOr(flags, FLAG_NONFINITE);
     p.w = tait_p_over_rho2(rho_new, ph);
     pos4[i] = p;
@@ -79,6 +82,50 @@ cudaError_t launch_download_pack(sph_ctx *c, float *pos3, float *vel3, float *rh
     if (n == 0) return cudaSuccess;
     download_pack_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(n, c->pos4[c->cur], c->velrho4[c->cur], c->acc4,
                                                                c->idt[c->cur], pos3, vel3, rho, acc3, drho);
+    c->n_launches++;
+    return cudaGetLastError();
+}
+
+// ---- exact checkpoint: the Verlet n-1 state in id order (particle data go to
+// the host "only when saving"; a saved run must continue on the same trajectory) -------------------
+__global__ void __launch_bounds__(256)
+m1_pack_kernel(uint32_t n, const float4 *__restrict__ velrhoM1, const uint32_t *__restrict__ idt,
+               float *__restrict__ vel3, float *__restrict__ rho)
+{
+    uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const uint32_t id = idt[i] & ID_MASK;
+    const float4 m = velrhoM1[i];
+    if (vel3) { vel3[3 * id] = m.x; vel3[3 * id + 1] = m.y; vel3[3 * id + 2] = m.z; }
+    if (rho) rho[id] = m.w;
+}
+
+cudaError_t launch_m1_pack(sph_ctx *c, float *vel3, float *rho)
+{
+    uint32_t n = (uint32_t)c->n;
+    if (n == 0) return cudaSuccess;
+    m1_pack_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(n, c->velrhoM1[c->cur], c->idt[c->cur], vel3, rho);
+    c->n_launches++;
+    return cudaGetLastError();
+}
+
+// live arrays are in id order (right after an upload): slot i holds particle i
+__global__ void __launch_bounds__(256)
+m1_unpack_kernel(uint32_t n, const float *__restrict__ vel3, const float *__restrict__ rho,
+                 float4 *__restrict__ velrhoM1, uint32_t *__restrict__ flags)
+{
+    uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const float4 m = make_float4(vel3[3 * i], vel3[3 * i + 1], vel3[3 * i + 2], rho[i]);
+    if (!(isfinite(m.x + m.y + m.z + m.w) && m.w > 0.f)) atomicOr(flags, FLAG_NONFINITE);
+    velrhoM1[i] = m;
+}
+
+cudaError_t launch_m1_unpack(sph_ctx *c, const float *vel3, const float *rho)
+{
+    uint32_t n = (uint32_t)c->n;
+    if (n == 0) return cudaSuccess;
+    m1_unpack_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(n, vel3, rho, c->velrhoM1[c->cur], c->flags);
     c->n_launches++;
     return cudaGetLastError();
 }

@@ -17,9 +17,13 @@ def make_sph(w, max_slabs=16, with_prev=True):
                  prev_slab=w.prev_slab if with_prev else None, max_slabs=max_slabs)
 
 
-def compare_structure(sph, w, planes, prev_slab, check_payload=True, check_halos=True):
+def compare_structure(sph, w, planes, prev_slab, check_payload=True, check_halos=True, check_halo_payload=None):
     """Bit-exact comparison of everything a1-a6 produce with ORACLE A on the generator's
-    inputs.  Returns the oracle dict."""
+    inputs.  Returns the oracle dict.  check_payload: the sorted state arrays carry w's bits;
+    check_halo_payload (default = check_payload): the halo buffers carry w's bits (they are copies
+    made BEFORE the Verlet update, so after sph_step they still hold the pre-step state)."""
+    if check_halo_payload is None:
+        check_halo_payload = check_payload
     P = w.params
     A = OA.structure(w.pos, np.arange(w.n), P["dom_min"], P["dom_max"], P["h"], planes, prev_slab)
     T = sph.view_tensors()
@@ -53,7 +57,7 @@ def compare_structure(sph, w, planes, prev_slab, check_payload=True, check_halos
                 exp = A["id_sorted"][A["halo"][s][side]]
                 got = hid[off[k]:off[k + 1]]
                 assert np.array_equal(got, exp.astype(np.uint32)), f"halo {s}/{side} membership differs"
-                if check_payload and len(exp):
+                if check_halo_payload and len(exp):
                     assert np.array_equal(hpos[off[k]:off[k + 1], :3].view(np.uint32), w.pos[exp].view(np.uint32))
                     assert np.array_equal(hvr[off[k]:off[k + 1], :3].view(np.uint32), w.vel[exp].view(np.uint32))
         mig = u32(T["migrants"]).astype(np.int64).reshape(-1, 4)
@@ -61,6 +65,38 @@ def compare_structure(sph, w, planes, prev_slab, check_payload=True, check_halos
         assert np.array_equal(mig, A["migrants"]), "migrant records differ"
         assert np.array_equal(u32(T["mig_count"]).astype(np.int64).reshape(S, 2), A["mig_count"])
     return A
+
+
+def owners_by_id(A, n):
+    """Owner slab of every particle id from an ORACLE A result."""
+    own = np.empty(n, dtype=np.uint8)
+    own[A["id_sorted"]] = A["slab_sorted"].astype(np.uint8)
+    return own
+
+
+def sampled_rate_errors(w, out, ids):
+    """Rates of the sampled particle ids against ORACLE B, which evaluates each sampled neighbourhood
+    (all particles within 2h per axis) by brute force.  Returns (worst_a, scale_a, worst_d, scale_d)."""
+    p = OB.params_from_workload(w.params)
+    two_h = 2.0 * w.params["h"]
+    worst_a = worst_d = scale_a = scale_d = 0.0
+    order = np.argsort(w.pos[:, 0], kind="stable")
+    xs = w.pos[order, 0]
+    for i in ids:
+        pi = w.pos[i].astype(np.float64)
+        lo = np.searchsorted(xs, np.float32(pi[0] - two_h * 1.01), side="left")
+        hi = np.searchsorted(xs, np.float32(pi[0] + two_h * 1.01), side="right")
+        cand = order[lo:hi]
+        sub = w.pos[cand].astype(np.float64)
+        near = np.sort(cand[(np.abs(sub - pi) <= two_h * 1.001).all(axis=1)])
+        k = int(np.nonzero(near == i)[0][0])
+        a, d = OB.rates(p, w.pos[near], w.vel[near], w.rho[near], w.type[near], mode=0)
+        if w.type[i] == 0:
+            worst_a = max(worst_a, np.abs(out["acc"][i] - a[k]).max())
+            scale_a = max(scale_a, np.abs(a[k]).max())
+        worst_d = max(worst_d, abs(out["drho"][i] - d[k]))
+        scale_d = max(scale_d, abs(d[k]))
+    return worst_a, scale_a, worst_d, scale_d
 
 
 def oracle_rates(w, kernel=None, mode=1):

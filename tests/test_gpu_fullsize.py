@@ -9,7 +9,7 @@ from oracle import physics as OB
 from oracle import structure as OA
 from paper_1210_1017_b200 import workloads as W
 
-from gpu_util import compare_structure, make_sph
+from gpu_util import compare_structure, make_sph, sampled_rate_errors
 
 pytestmark = pytest.mark.gpu
 
@@ -27,25 +27,86 @@ def test_config3_full_size_structure_and_sampled_rates():
     sph.sph_interact()
     out = sph.sph_download(pos=False, vel=False, rho=False)
     assert sph.sph_status() == 0
-    p = OB.params_from_workload(w.params)
-    ids = (W.u01(317, np.arange(24), 0) * w.n).astype(np.int64)
-    two_h = 2.0 * w.params["h"]
-    worst_a = worst_d = scale_a = scale_d = 0.0
-    for i in ids:
-        pi = w.pos[i].astype(np.float64)
-        # cheap pre-selection on x, then the box test on the survivors
-        cand = np.nonzero(np.abs(w.pos[:, 0] - np.float32(pi[0])) <= np.float32(two_h * 1.01))[0]
-        sub = w.pos[cand].astype(np.float64)
-        near = cand[(np.abs(sub - pi) <= two_h * 1.001).all(axis=1)]
-        k = int(np.nonzero(near == i)[0][0])
-        a, d = OB.rates(p, w.pos[near], w.vel[near], w.rho[near], w.type[near], mode=0)
-        if w.type[i] == 0:
-            worst_a = max(worst_a, np.abs(out["acc"][i] - a[k]).max())
-            scale_a = max(scale_a, np.abs(a[k]).max())
-        worst_d = max(worst_d, abs(out["drho"][i] - d[k]))
-        scale_d = max(scale_d, abs(d[k]))
+    ids = _sample_ids(w, planes, nc, 128, 64, 32, 64)
+    assert len(ids) >= 256
+    worst_a, scale_a, worst_d, scale_d = sampled_rate_errors(w, out, ids)
     assert scale_a > 0 and scale_d > 0
     assert worst_a <= 1e-4 * scale_a and worst_d <= 1e-4 * scale_d
+
+
+def _sample_ids(w, planes, nc, n_random, n_wall, n_bound, n_plane):
+    """Sampled particle ids: random ones, fluid particles on the faces of the block (their cells also
+    hold boundary particles), boundary particles, and fluid particles next to the slab planes."""
+    nb = w.notes["nb"]
+    nf = w.n_fluid
+    dp = w.params["dp"]
+    ids = list((W.u01(317, np.arange(n_random), 0) * w.n).astype(np.int64))
+    r = (W.u01(318, np.arange(3 * n_wall), 0) * nb).astype(np.int64).reshape(-1, 3)
+    for q, (a, b, c) in enumerate(r):
+        face = q % 5
+        i, j, k = [(0, a, b), (a, 0, b), (a, b, 0), (nb - 1, a, b), (a, nb - 1, b)][face]
+        ids.append((i * nb + j) * nb + k)
+    ids += list(nf + (W.u01(319, np.arange(n_bound), 0) * (w.n - nf)).astype(np.int64))
+    cell = 2.0 * w.params["h"]
+    inner = [p for p in planes[1:-1] if 0 < (w.params["dom_min"][0] + p * cell) / dp < nb - 1]
+    assert inner
+    r = (W.u01(320, np.arange(2 * n_plane), 0) * nb).astype(np.int64).reshape(-1, 2)
+    for q, (a, b) in enumerate(r):
+        xp = w.params["dom_min"][0] + inner[q % len(inner)] * cell
+        i = min(max(int(np.floor(xp / dp)) - (q // len(inner)) % 2, 0), nb - 1)   # lattice layer right / left of the plane
+        ids.append((i * nb + a) * nb + b)
+    return np.unique(np.asarray(ids, dtype=np.int64))
+
+
+def test_config2_full_size_structure_and_sampled_rates():
+    """BASELINE config 2 (8.8 M particles, 8 slabs) at full size: complete structure comparison and
+    the rates of >= 64 sampled particles."""
+    w = W.dam_break(200, scrambled=True)
+    assert w.n == 8824704
+    nc = OA.grid_dims(w.params["dom_min"], w.params["dom_max"], w.params["h"])
+    planes = W.slab_planes(nc[0], 8)
+    sph = make_sph(w)
+    sph.sph_set_slabs(planes)
+    sph.sph_sort_and_cells()
+    sph.sph_build_halos()
+    compare_structure(sph, w, planes, None)
+    sph.sph_interact()
+    out = sph.sph_download(pos=False, vel=False, rho=False)
+    assert sph.sph_status() == 0
+    ids = _sample_ids(w, planes, nc, 32, 24, 12, 24)
+    assert len(ids) >= 64
+    worst_a, scale_a, worst_d, scale_d = sampled_rate_errors(w, out, ids)
+    assert scale_a > 0 and scale_d > 0
+    assert worst_a <= 1e-4 * scale_a and worst_d <= 1e-4 * scale_d
+
+
+def test_config3_full_size_ten_steps():
+    """BASELINE config 3 (33.9 M particles, 16 slabs rebuilt every step), scrambled start: state after
+    10 Verlet steps against ORACLE B stepping the same 10 steps in fp64 (relative L2 <= 1e-3 on r, v,
+    rho and on the displacement)."""
+    from gpu_util import rel_l2
+    w = W.dam_break(317, scrambled=True)
+    nc = OA.grid_dims(w.params["dom_min"], w.params["dom_max"], w.params["h"])
+    sph = make_sph(w, with_prev=False)
+    sph.sph_set_slabs(W.slab_planes(nc[0], 16))
+    for _ in range(10):
+        sph.sph_step(w.dt)
+    out = sph.sph_download(acc=False, drho=False)
+    assert sph.sph_status() == 0
+    sph.sph_destroy()
+    del sph
+    p = OB.params_from_workload(w.params)
+    s = OB.State(w.pos, w.vel, w.rho, w.type)
+    for _ in range(10):
+        OB.step(p, s, w.dt, verlet_ns=w.params["verlet_ns"])
+    fl = w.type == 0
+    assert rel_l2(out["pos"], s.r) <= 1e-3
+    assert rel_l2(out["rho"], s.rho) <= 1e-3
+    assert rel_l2(out["vel"][fl], s.v[fl]) <= 1e-3
+    disp_ref = s.r[fl] - w.pos[fl].astype(np.float64)
+    disp = out["pos"][fl].astype(np.float64) - w.pos[fl].astype(np.float64)
+    assert np.linalg.norm(disp - disp_ref) <= 1e-3 * np.linalg.norm(disp_ref)
+    assert np.array_equal(out["pos"][~fl], w.pos[~fl])
 
 
 def test_config1_full_size_ten_steps():

@@ -143,3 +143,56 @@ def test_micro_16m_structure_properties_and_samples():
     sph.sph_sort_and_cells()
     sph.sph_build_halos()
     compare_structure(sph, w, planes, w.prev_slab, check_payload=False)
+
+
+def test_micro_64m_full_structure():
+    """Sort/halo microbenchmark size 2^26 (3 radix passes at full tile counts): the complete structure
+    comparison (numpy lexsort of 67 M keys)."""
+    w = W.uniform_cube(1 << 26)
+    planes = _planes(w, 8)
+    sph = make_sph(w)
+    sph.sph_set_slabs(planes)
+    sph.sph_sort_and_cells()
+    sph.sph_build_halos()
+    compare_structure(sph, w, planes, w.prev_slab, check_payload=False)
+
+
+def test_micro_256m_four_pass_sort_by_its_defining_properties():
+    """2^28 particles, 26 key bits = 4 radix passes at full tile counts.  Instead of a 268 M-element
+    lexsort the result is checked through the three properties that define it uniquely: (i) the ids are
+    a permutation, (ii) every sorted keyword is ORACLE A's keyword of that id, (iii) the sequence is
+    strictly increasing in (cell, id).  The cell table is checked against searchsorted on the (then
+    proven) sorted cells, the slab ranges against it."""
+    n = 1 << 28
+    w = W.uniform_cube(n)
+    P = w.params
+    planes = _planes(w, 8)
+    sph = make_sph(w)
+    v = sph.sph_get_view()
+    assert v.cell_bits == 26
+    sph.sph_set_slabs(planes)
+    sph.sph_sort_and_cells()
+    sph.sph_build_halos()
+    assert sph.sph_status() == 0
+    T = sph.view_tensors()
+    kw = u32(T["keyword"])
+    ids = (u32(T["idt"]) & 0x0FFFFFFF).astype(np.int64)
+    assert np.array_equal(np.bincount(ids, minlength=n), np.ones(n, dtype=np.int64))            # (i)
+    nc = OA.grid_dims(P["dom_min"], P["dom_max"], P["h"])
+    kw_by_id, cell_by_id = OA.keywords(w.pos, P["dom_min"], P["h"], nc, planes, w.prev_slab)
+    assert np.array_equal(kw, kw_by_id[ids])                                                    # (ii)
+    cell = (kw & 0x0FFFFFFF).astype(np.int64)
+    comp = cell * n + ids                                                                       # < 2^54
+    assert (np.diff(comp) > 0).all()                                                            # (iii)
+    del comp, kw_by_id, cell_by_id
+    ncells = nc[0] * nc[1] * nc[2]
+    begin, _ = OA.cell_table(cell, ncells)
+    assert np.array_equal(u32(T["cell_begin"]), begin)
+    assert np.array_equal(u32(T["slab_begin"]), begin[np.asarray(planes, dtype=np.int64) * nc[1] * nc[2]])
+    # migrants: count and records against the linear filter over the sorted sequence
+    slab_s = OA.slab_of(cell // (nc[1] * nc[2]), planes)
+    prev_s = w.prev_slab[ids].astype(np.int64)
+    m = np.nonzero(prev_s != slab_s)[0]
+    mig = u32(T["migrants"]).astype(np.int64).reshape(-1, 4)
+    assert len(mig) == len(m) > 0
+    assert np.array_equal(mig, np.stack([ids[m], m, prev_s[m], slab_s[m]], axis=1))

@@ -53,7 +53,26 @@ def test_grid_dims_configs():
     """2h = 3dp cells; config 0 tank 0.4x0.2x0.3 with a 5dp margin each side: 50/25/35 dp."""
     w = W.dam_break(16)
     nc = OA.grid_dims(w.params["dom_min"], w.params["dom_max"], w.params["h"])
-    assert nc == (17, 9, 14) or nc == (17, 10, 14) or nc[0] in (17, 18)
+    # hand derivation: extent = tank + 2 (2 dp + 2h) = tank + 10 dp, cell = 3 dp.  The number of cells
+    # is ceil(extent / cell); where the real quotient is an integer the fp32 rounding of the
+    # parameters decides between q and q + 1 (both listed), elsewhere the value is forced.
+    hand = {  # nb: per axis (extent in dp, forced value or the two candidates)
+        16: ((50.0, (17,)), (30.0, (10, 11)), (40.0, (14,))),                      # 16.67, 10, 13.33
+        100: ((310.0, (104,)), (135.625, (46,)), (110.0, (37,))),                 # 103.33, 45.2, 36.67
+        200: ((610.0, (204,)), (261.25, (88,)), (210.0, (70, 71))),               # 203.33, 87.08, 70
+        317: ((961.0, (321,)), (408.23125, (137,)), (327.0, (109, 110))),         # 320.33, 136.08, 109
+    }
+    exact = {16: (17, 11, 14), 100: (104, 46, 37), 200: (204, 88, 70), 317: (321, 137, 110)}
+    for nb, axes in hand.items():
+        P = W.dam_break_params(nb)
+        got = OA.grid_dims(P["dom_min"], P["dom_max"], P["h"])
+        for k, (ext_dp, allowed) in enumerate(axes):
+            q = ext_dp / 3.0
+            if abs(q - round(q)) > 1e-6:
+                assert allowed == (math.ceil(q),)
+            assert got[k] in allowed, (nb, k, got)
+        assert got == exact[nb]
+    assert nc == exact[16]
     # every particle of the config lies strictly inside the grid (no clamping active)
     inv = 1.0 / (2.0 * w.params["h"])
     t = (w.pos.astype(np.float64) - np.array(w.params["dom_min"])) * inv
@@ -194,3 +213,73 @@ def test_first_call_has_no_migrants_and_single_slab_no_edges():
     # lattice sanity: 2h = 3dp, so an interior fluid cell holds 27 particles
     occ = np.diff(A["cell_begin"].astype(np.int64))
     assert occ.max() == 27
+
+
+# ---------------------------------------------------------------- movable slab planes (NEXT-4)
+def test_balance_planes_uniform_counts_give_even_planes():
+    """Equal counts per plane: the balanced planes are the evenly spaced ones."""
+    assert OA.balance_planes([5] * 24, 4) == [0, 6, 12, 18, 24]
+    assert OA.balance_planes([1] * 16, 8) == [0, 2, 4, 6, 8, 10, 12, 14, 16]
+    assert OA.balance_planes([7] * 9, 1) == [0, 9]
+
+
+def test_balance_planes_hand_cases():
+    # all particles in the first two planes: planes are pushed right only as far as ">= 2 planes
+    # per slab" forces them; ties (empty planes all cost the same) go to the LOWEST plane
+    assert OA.balance_planes([10, 10, 0, 0, 0, 0, 0, 0], 2) == [0, 2, 8]        # C[2] = 20 > 10: |40 - 20| = 20 at p = 2..6, lowest wins
+    # C = 0 1 2 3 103 104 105 106 107; N = 107; S = 2: target 53.5 -> |2C - 107|: p=3: 101, p=4: 99 -> 4
+    assert OA.balance_planes([1, 1, 1, 100, 1, 1, 1, 1], 2) == [0, 4, 8]
+    # three slabs, dam-break-like: fluid in the left third
+    counts = [0, 9, 9, 9, 9, 1, 1, 1, 1, 1, 1, 0]
+    pl = OA.balance_planes(counts, 3)
+    assert pl == [0, 3, 5, 12]          # N = 42: targets 14, 28; C = 0 0 9 18 27 36 37 ..: |3C - 42| min at p = 3 (12); then |3C - 84| min at p = 5 (24 vs p = 4: 3)
+    # ... the second plane: C[4] = 27 -> |81 - 84| = 3 but p must be >= 3 + 2 = 5 -> C[5] = 36 -> 24
+
+
+def test_balance_planes_brute_force_is_locally_optimal():
+    """Each interior plane, given its left neighbour, is the feasible plane closest to its target
+    (pure-python search); planes are feasible; the spread of the owned counts never gets worse than
+    with evenly spaced planes on a one-sided distribution."""
+    rng_counts = (W.u01(77, np.arange(60), 0) ** 3 * 1000).astype(np.int64)
+    for S in (2, 3, 5, 8):
+        pl = OA.balance_planes(rng_counts, S)
+        assert OA.check_planes(pl, 60)
+        C = np.concatenate([[0], np.cumsum(rng_counts)])
+        N = int(C[-1])
+        for s in range(1, S):
+            lo, hi = pl[s - 1] + 2, 60 - 2 * (S - s)
+            costs = {p: abs(int(C[p]) * S - s * N) for p in range(lo, hi + 1)}
+            m = min(costs.values())
+            assert pl[s] == min(p for p, c in costs.items() if c == m)
+        owned = np.diff(C[pl])
+        even = np.diff(C[W.slab_planes(60, S)])
+        assert owned.max() <= even.max()
+
+
+def test_plane_counts_sum_and_match_structure():
+    w = W.dam_break(16)
+    P = w.params
+    cnt = OA.plane_counts(w.pos, P["dom_min"], P["dom_max"], P["h"])
+    assert cnt.sum() == w.n
+    nc = OA.grid_dims(P["dom_min"], P["dom_max"], P["h"])
+    pl = OA.balance_planes(cnt, 3)
+    A = OA.structure(w.pos, np.arange(w.n), P["dom_min"], P["dom_max"], P["h"], pl)
+    assert A["owned"].sum() == w.n
+    B = OA.structure(w.pos, np.arange(w.n), P["dom_min"], P["dom_max"], P["h"], W.slab_planes(nc[0], 3))
+    assert A["owned"].max() < B["owned"].max()          # the fluid sits in the left part of the tank
+
+
+def test_neighbour_pairs_counts_on_an_integer_lattice():
+    """Pin of the brute-force neighbour list: unit lattice, h = 1.5 (2h = 3).  Integer vectors with
+    0 < |v|^2 < 9: r3(1..8) = 6 + 12 + 8 + 6 + 24 + 24 + 0 + 12 = 92; another r3(9) = 30 sit exactly AT
+    r = 2h and count only when the cut-off is a hair larger (strict inequality)."""
+    r = W.lattice_block(9, 9, 9, 1.0)
+    centre = (4 * 9 + 4) * 9 + 4
+    pairs = OB.neighbour_pairs(OB.make_params(h=1.5), r)
+    assert np.count_nonzero(pairs[:, 0] == centre) == 92
+    assert np.count_nonzero(pairs[:, 1] == centre) == 92                 # symmetric
+    assert len(set(map(tuple, pairs))) == len(pairs) and (pairs[:, 0] != pairs[:, 1]).all()
+    pairs = OB.neighbour_pairs(OB.make_params(h=1.5 * (1 + 1e-9)), r)
+    assert np.count_nonzero(pairs[:, 0] == centre) == 122
+    corner = OB.neighbour_pairs(OB.make_params(h=0.5 * (1 + 1e-9)), r)   # 2h = 1+: face neighbours only
+    assert np.count_nonzero(corner[:, 0] == 0) == 3 and np.count_nonzero(corner[:, 0] == centre) == 6
