@@ -110,6 +110,8 @@ cudaError_t launch_interact_slab(sph_ctx *c, int s, const uint32_t *h_slab_begin
     c->ia_ov.acc4 = acc_loc - base;
     c->ia_ov.cx_first = c->tagged_slabs.planes[s];
     c->ia_ov.cx_count = c->tagged_slabs.planes[s + 1] - c->tagged_slabs.planes[s];
+    c->ia_ov.cand_lo = p_lo;
+    c->ia_ov.cand_hi = p_hi;
     const int variant = c->interact_variant;
     c->interact_variant = 0;
     e = launch_interact(c, false);

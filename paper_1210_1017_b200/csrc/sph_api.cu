@@ -313,6 +313,11 @@ int sph_init(sph_ctx **out, const sph_params *p, const sph_particles *part, int 
     if (zb < 1) zb = 1;
     if (zb > 32) zb = 32;
     c->zblock = zb;
+    // production kernel: a tile of 2 x 2 columns x zm cells fills the CTA's threads with targets
+    int zm = (int)floor((double)interact_mma_threads() * 0.97 / (4.0 * (ppc > 0.05 ? ppc : 0.05)));
+    if (zm < 1) zm = 1;
+    if (zm > interact_mma_zmax()) zm = interact_mma_zmax();
+    c->zblock_mma = zm;
 
     c->last_cuda_error[0] = 0;
     c->id_order = true;

@@ -55,6 +55,7 @@ struct IaOverride {
     const uint32_t *idt, *keyword, *cell_begin;
     float4 *acc4;
     int cx_first, cx_count;      // cell planes [cx_first, cx_first + cx_count) hold the targets
+    int cand_lo, cand_hi;        // cell planes that exist in the local arrays (own + halo planes), inclusive
 };
 
 // ---- profiling ------------------------------------------------------------------------
@@ -123,7 +124,8 @@ struct sph_ctx {
     int adaptive_dt;           // SPH_OPT_ADAPTIVE_DT: sph_interact also produces mumax
     uint64_t step_index;
     int interact_variant;
-    int zblock;                // cells per z-block of the staged interaction kernel
+    int zblock;                // cells per z-block of the staged (round-1) interaction kernel
+    int zblock_mma;            // cells per z-block of a tile of the production interaction kernel
 
     uint64_t n_launches;       // kernels launched so far (memsets and copies not counted)
     bool id_order;             // live state arrays are still in id order (no sort since the last upload)
@@ -162,6 +164,10 @@ cudaError_t launch_balance(sph_ctx *c, int n_slabs, int32_t *d_planes);
 cudaError_t launch_fma_peak(sph_ctx *c, int variant, int iters, int blocks, float *sink);
 // per-device kernel attributes (dynamic shared memory opt-in), set for every new context
 cudaError_t configure_interact();
+cudaError_t configure_interact_mma();
+cudaError_t launch_interact_mma(sph_ctx *c, bool with_mu);
+int interact_mma_threads();
+int interact_mma_zmax();
 cudaError_t configure_sort();
 
 uint32_t radix_tiles(uint64_t n);

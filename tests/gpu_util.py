@@ -129,3 +129,13 @@ def rel_l2(got, ref):
     d = np.linalg.norm(got.astype(np.float64) - ref)
     s = np.linalg.norm(ref)
     return d / s if s > 0 else d
+
+
+def position_rounding_floor(pos0_fluid, n_steps):
+    """Expected L2 norm of the rounding noise that fp32 POSITIONS pick up in n_steps Verlet updates:
+    r+ = fma(dt^2/2, a, fma(dt, v, r)) rounds twice per step at the magnitude of r, each rounding error
+    uniform in +-ulp(r)/2 (variance ulp^2/12).  No fp32-state implementation can follow the fp64 oracle's
+    DISPLACEMENT more closely than this; it matters where displacements are small against the
+    coordinates (config 3: 10 steps move a particle ~3e-5 m at x ~ 0.5 m, ulp = 6e-8 m).  DESIGN.md 2."""
+    ulp = np.spacing(np.abs(np.asarray(pos0_fluid, dtype=np.float32))).astype(np.float64)
+    return float(np.sqrt(2.0 * n_steps * np.sum(ulp * ulp) / 12.0))

@@ -163,7 +163,12 @@ def test_dam_break_rebalanced_every_20_steps():
             planes = new
             prev = owners_by_id(A2, w.n)
             sph.sph_step(w.dt)                            # its sort sees unmoved particles: no migrants
-            prev_after = prev
+        elif k % 20 == 19:
+            # the owners the next re-balance compares with are those of THIS step's sort
+            pos, _, _ = _state(sph)
+            sph.sph_step(w.dt)
+            cx, _, _ = OA.cell_coords(pos, P["dom_min"], P["h"], nc)
+            prev = OA.slab_of(cx, planes).astype(np.uint8)
         else:
             sph.sph_step(w.dt)
     assert sph.sph_status() == 0
