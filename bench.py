@@ -34,9 +34,11 @@ CONFIG_NB = {0: 16, 1: 100, 2: 200, 3: 317}
 METRIC = "Mparticle-steps/s"
 FP32_LANES_PER_SM, NUM_SMS = 128, 148
 FLOPS_PER_CANDIDATE, FLOPS_PER_PAIR = 8, 32
-# dram__bytes_read.sum + dram__bytes_write.sum of one interact_staged_kernel launch at config 3
-# (profiles/r01_ncu_full_config3_v4.md); other configs have no capture
-IA_TRAFFIC_BYTES = {3: 1.379577e9 + 0.529622e9}
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the production interaction kernel, from
+# an `ncu --set full` capture of this command (DRAM counters cannot be read inside a timed run): config ->
+# (bytes, file under profiles/ that holds the capture).  Configs without a capture report null.
+IA_TRAFFIC = {}
+IA_KERNEL = {0: "interact_mma_kernel", 1: "interact_simple_kernel", 2: "interact_staged_kernel"}
 # algorithmic HBM bytes per particle of the memory-bound stages
 BYTES = dict(keys=28.0, sort_per_pass=16.0, gather=116.0, verlet=116.0, migrate=4.0)
 
@@ -123,7 +125,39 @@ def oracle_step_sample(w, max_particles: int):
     OA.structure(pos, np.arange(len(sel)), P["dom_min"], P["dom_max"], P["h"], planes)
     OB.step(p, s, w.dt, verlet_ns=P["verlet_ns"])
     dt = time.perf_counter() - t0
-    return len(sel), dt, OB.threads(), f"{len(sel)} particles of lowest x of {w.name}, 1 step (structure + rates + Verlet)"
+    desc = f"{len(sel)} particles of lowest x of {w.name}, 1 step (structure + rates + Verlet)"
+    if n < w.n:
+        desc += " - a wall-heavy end of the tank: see mean_neighbours against the whole workload's"
+    return len(sel), dt, OB.threads(), desc
+
+
+def mean_neighbours(pos, h, probes: int = 20000) -> float:
+    """Descriptive statistic only (scipy k-d tree, not the oracle): mean number of neighbours with
+    0 < r < 2h of `probes` evenly spaced particles of the set."""
+    from scipy.spatial import cKDTree
+    tree = cKDTree(pos.astype(np.float64))
+    sel = np.linspace(0, len(pos) - 1, min(probes, len(pos))).astype(np.int64)
+    cnt = tree.query_ball_point(pos[sel].astype(np.float64), 2.0 * h * (1.0 - 1e-12), return_length=True)
+    return float(np.mean(cnt) - 1.0)
+
+
+def oracle_sample_neighbours(w, max_particles: int) -> float:
+    n = min(w.n, max_particles)
+    if n < w.n:
+        xs = np.partition(w.pos[:, 0], n - 1)[n - 1]
+        sel = np.nonzero(w.pos[:, 0] <= xs)[0][:n]
+        return mean_neighbours(w.pos[sel], w.params["h"])
+    return mean_neighbours(w.pos, w.params["h"])
+
+
+def oracle_structure_sample(w, planes):
+    """Oracle A (structure definition: keys, sort, cell table, slab ranges, halos, migrants), as it
+    stands, on the whole workload.  Returns seconds."""
+    from oracle import structure as OA
+    P = w.params
+    t0 = time.perf_counter()
+    OA.structure(w.pos, np.arange(w.n), P["dom_min"], P["dom_max"], P["h"], planes, prev_slab=w.prev_slab)
+    return time.perf_counter() - t0
 
 
 def run_reference(args):
@@ -146,12 +180,33 @@ def run_reference(args):
     line = dict(impl="reference", metric=METRIC, value=value, unit="Mparticle-steps/s", n_gpus=args.gpus,
                 steps=args.steps, warmup=args.warmup, ms_per_step=1e3 * t / args.steps,
                 higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64", data="synthetic",
-                config=dict(workload=f"config{args.config}: {w.name}", n_particles=w.n, n_slabs=w.n_slabs,
-                            sample=desc),
+                config=dict(workload=f"config{args.config}: {w.name}", n_particles=n_s, sampled=True,
+                            n_particles_of_workload=w.n, n_slabs=w.n_slabs, sample=desc),
                 cpu_baseline=dict(value=value, unit="Mparticle-steps/s", cores=cores, kind="oracle", sample=desc),
                 e2e=dict(value=value, unit="Mparticle-steps/s", h2d_bytes_per_step=0, d2h_bytes_per_step=0),
                 gpu_launches=0)
     print(json.dumps(line))
+
+
+def migrate_bytes(n: int, n_mig: int) -> float:
+    """Algorithmic bytes of the migrant compaction: the keyword of every slot of a 4096-slot group that
+    holds a migrant (groups without one are skipped: their count was taken by the gather kernel) +
+    16 B per record written."""
+    return min(4.0 * n, 4.0 * 4096 * n_mig) + 16.0 * n_mig
+
+
+def stage_entry(ms: float, nbytes, hbm_gbs: float, **extra) -> dict:
+    """One HBM-bound stage: algorithmic GB/s and fraction of the measured copy peak.  A stage that moved
+    less than 1 MB (no migrants, tiny halo planes) is launch latency, not a bandwidth: null."""
+    d = dict(ms=ms, **extra)
+    if nbytes is None:
+        return d
+    if nbytes < 1e6:
+        d.update(algorithmic_gbs=None, frac_of_hbm_peak=None, note="< 1 MB moved: launch latency, not a bandwidth")
+        return d
+    gbs = nbytes / (ms * 1e-3) / 1e9
+    d.update(algorithmic_gbs=gbs, frac_of_hbm_peak=gbs / hbm_gbs)
+    return d
 
 
 def run_micro(args):
@@ -186,21 +241,26 @@ def run_micro(args):
     passes = (v.cell_bits + 7) // 8
     med = {k: float(np.median(x)) for k, x in acc.items() if np.sum(x) > 0}
     byts = dict(keys=BYTES["keys"] * n, sort=BYTES["sort_per_pass"] * passes * n, gather=BYTES["gather"] * n,
-                cells=None, halo=72.0 * n_halo, migrate=4.0 * n + 16.0 * n_mig)
+                cells=None, halo=72.0 * n_halo, migrate=migrate_bytes(n, n_mig))
     out = dict(workload=w.name, n=n, cell_bits=v.cell_bits, passes=passes, n_halo=n_halo, n_migrants=n_mig,
                sort_gkeys_s=n / (med["sort"] * 1e-3) / 1e9,
                sort_with_keys_gkeys_s=n / ((med["sort"] + med["keys"]) * 1e-3) / 1e9,
                hbm_peak_gbs=pk["hbm_gbs"], peak_source=pk["source"],
-               stages={k: (dict(ms=med[k], algorithmic_gbs=byts[k] / (med[k] * 1e-3) / 1e9,
-                                frac_of_hbm_peak=byts[k] / (med[k] * 1e-3) / 1e9 / pk["hbm_gbs"])
-                           if byts[k] is not None else dict(ms=med[k]))
-                       for k in med if k in byts})
+               stages={k: stage_entry(med[k], byts[k], pk["hbm_gbs"]) for k in med if k in byts})
+    ks_b = byts["keys"] + byts["sort"]
+    ks_ms = med["keys"] + med["sort"]
+    out["stages"]["keys+sort"] = stage_entry(ks_ms, ks_b, pk["hbm_gbs"])
+    if not args.no_cpu_baseline and args.micro <= 26:
+        # structure cpu_baseline: Oracle A (numpy; lexsort, searchsorted and filters are single-threaded)
+        sec = oracle_structure_sample(w, planes)
+        out["cpu_baseline"] = dict(value=n / sec / 1e6, unit="Mkeys/s (structure: keys, sort, cell table, halos, "
+                                   "migrants)", cores=1, kind="oracle", seconds=sec,
+                                   sample=f"all {n} particles of {w.name}, one structure build")
     # the cell table is written by the gather kernel (short gaps) and the gap-fill kernel of the
     # "cells" stage (long runs of empty cells): one combined figure, 4 B written per cell
     gc_ms = med["gather"] + med["cells"]
     gc_b = byts["gather"] + 4.0 * (v.ncells + 1)
-    out["stages"]["gather+cells"] = dict(ms=gc_ms, algorithmic_gbs=gc_b / (gc_ms * 1e-3) / 1e9,
-                                         frac_of_hbm_peak=gc_b / (gc_ms * 1e-3) / 1e9 / pk["hbm_gbs"])
+    out["stages"]["gather+cells"] = stage_entry(gc_ms, gc_b, pk["hbm_gbs"])
     print(json.dumps(out))
 
 
@@ -218,6 +278,9 @@ def main():
     ap.add_argument("--ref-sample", type=int, default=300_000, help="particles per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--variant", type=int, default=0)
+    ap.add_argument("--disorder", type=int, default=0, metavar="K",
+                    help="time a DISORDERED fluid instead of the rest-state lattice: scrambled start (random "
+                         "velocities 0.1 sqrt(gH), densities rho0 (1 + U(0, 1 %%))) stepped K times before warm-up")
     ap.add_argument("--adaptive", action="store_true", help="timed steps use sph_step_adaptive(cfl = 0.2) (variable dt)")
     args = ap.parse_args()
     if args.steps is None:
@@ -244,7 +307,7 @@ def main():
     pk = peaks()
 
     nb = CONFIG_NB[args.config]
-    w = W.dam_break(nb)
+    w = W.dam_break(nb, scrambled=args.disorder > 0)
     sph = B.Sph(w.params, w.pos, w.vel, w.rho, w.type, device=f"cuda:{local}")
     sph.sph_set_option(B.SPH_OPT_INTERACT_VARIANT, args.variant)
     v = sph.sph_get_view()
@@ -256,7 +319,9 @@ def main():
     def barrier():
         R.barrier(rep)
 
-    # ---- warm-up
+    # ---- warm-up (preceded by the steps that let a scrambled start disorder the lattice)
+    for _ in range(args.disorder):
+        sph.sph_step(w.dt)
     for _ in range(args.warmup):
         sph.sph_step(w.dt)
     assert sph.sph_status() == 0
@@ -312,7 +377,7 @@ def main():
     e2e_single = world * n * args.e2e_steps / e2e_single_s / 1e6
     # (b) several contexts (default 3) on their own streams, one host thread each: the same three calls per step,
     # but one context's PCIe copies overlap the other's kernels (what a user with a queue of
-    # independent jobs does).  This is the reported end-to-end value; (a) is printed beside it.
+    # independent jobs does).  (a) is the reported end-to-end value; (b) is printed beside it.
     e2e_value, e2e_ctx = e2e_single, 1
     if args.e2e_steps > 0 and args.e2e_contexts > 1:
         import threading
@@ -346,11 +411,15 @@ def main():
         e2e_ctx = len(ctxs)
         for c2 in ctxs[1:]:
             c2.sph_destroy()
-    e2e = dict(value=e2e_value, unit="Mparticle-steps/s",
+    # e2e.value = ONE simulation: upload, step, download strictly one after the other.  The figure of
+    # several independent simulations sharing the GPU (copies of one overlap the kernels of another) is
+    # printed beside it under its own key.
+    e2e = dict(value=e2e_single, unit="Mparticle-steps/s",
                h2d_bytes_per_step=int(n * (12 + 12 + 4 + 1)), d2h_bytes_per_step=int(n * (12 + 12 + 4)),
-               steps=args.e2e_steps * e2e_ctx, contexts=e2e_ctx, single_context_value=e2e_single,
-               api="per step: sph_set_state(host) + sph_step + sph_download(host), pinned buffers; "
-                   f"{e2e_ctx} context(s) on separate streams so copies overlap kernels")
+               steps=args.e2e_steps, contexts=1,
+               api="per step: sph_set_state(host) + sph_step + sph_download(host), pinned buffers, one context",
+               pipelined=dict(value=e2e_value, contexts=e2e_ctx, steps=args.e2e_steps * e2e_ctx,
+                              note=f"{e2e_ctx} independent simulations on separate streams, one host thread each"))
 
     if rank != 0:
         R.finalize(rep)
@@ -363,9 +432,14 @@ def main():
     achieved = flops / (ia_ms_avg * 1e-3) / 1e12
     peak = NUM_SMS * FP32_LANES_PER_SM * 2 * pk["sm_max_mhz"] * 1e6 / 1e12
     sm_mhz = clocks.get("sm_mhz") or pk["sm_max_mhz"]
-    roofline = dict(bound="alu", kernel="interact_staged_kernel", achieved=achieved, peak=peak, unit="TFLOP/s",
-                    frac=achieved / peak, traffic=IA_TRAFFIC_BYTES.get(args.config),
+    # the FP32 peak this box really sustains: register-resident FMA chains, same process (csrc/fma_peak.cu)
+    peak_meas = max(sph.sph_fma_peak(0, 8192), sph.sph_fma_peak(1, 8192))
+    traffic, traffic_src = IA_TRAFFIC.get(args.config if not args.disorder else None, (None, None))
+    roofline = dict(bound="alu", kernel=IA_KERNEL.get(args.variant, "?"), achieved=achieved, peak=peak, unit="TFLOP/s",
+                    frac=achieved / peak, traffic=traffic, traffic_source=traffic_src,
                     peak_source=f"148 SMs x 128 FP32 lanes x 2 flop x {pk['sm_max_mhz']:.0f} MHz (max clock, {pk['source']})",
+                    peak_measured=peak_meas, frac_of_measured_peak=achieved / peak_meas,
+                    peak_measured_source="sph_fma_peak: FFMA / FFMA2 chains in registers, best of the two, this run",
                     frac_at_observed_clock=achieved / (peak * sm_mhz / pk["sm_max_mhz"]),
                     algorithmic_flops_per_launch=flops, candidates=cand, pairs=pairs,
                     avg_launch_ms=ia_ms_avg, share_of_step=ia_ms / ms_total)
@@ -374,30 +448,28 @@ def main():
     n_halo = int(T["halo_offset"][-1].item()) if w.n_slabs > 1 else 0
     n_mig = int(T["mig_total"].item())
     byts = dict(keys=BYTES["keys"] * n, sort=BYTES["sort_per_pass"] * passes * n, gather=BYTES["gather"] * n,
-                cells=None, halo=72.0 * n_halo, migrate=4.0 * n + 16.0 * n_mig,
+                cells=None, halo=72.0 * n_halo, migrate=migrate_bytes(n, n_mig),
                 verlet=BYTES["verlet"] * n)
     stages = {}
     for k, (ms, c) in stage.items():
         if c == 0:
             continue
-        avg = ms / c
-        d = dict(ms=avg, share=ms / ms_total)
-        if byts.get(k) is not None:
-            gbs = byts[k] / (avg * 1e-3) / 1e9
-            d.update(algorithmic_gbs=gbs, frac_of_hbm_peak=gbs / pk["hbm_gbs"])
-        stages[k] = d
+        stages[k] = stage_entry(ms / c, byts.get(k), pk["hbm_gbs"], share=ms / ms_total)
     if "gather" in stages and "cells" in stages:      # see run_micro: one combined figure for a3 + a4
         gc_ms = stages["gather"]["ms"] + stages["cells"]["ms"]
         gc_b = byts["gather"] + 4.0 * (v.ncells + 1)
-        stages["gather+cells"] = dict(ms=gc_ms, share=gc_ms * args.steps / ms_total,
-                                      algorithmic_gbs=gc_b / (gc_ms * 1e-3) / 1e9,
-                                      frac_of_hbm_peak=gc_b / (gc_ms * 1e-3) / 1e9 / pk["hbm_gbs"])
+        stages["gather+cells"] = stage_entry(gc_ms, gc_b, pk["hbm_gbs"], share=gc_ms * args.steps / ms_total)
+    if "keys" in stages and "sort" in stages:
+        ks_ms = stages["keys"]["ms"] + stages["sort"]["ms"]
+        stages["keys+sort"] = stage_entry(ks_ms, byts["keys"] + byts["sort"], pk["hbm_gbs"],
+                                          share=ks_ms * args.steps / ms_total)
     cpu = None
     if not args.no_cpu_baseline:
         oracle_step_sample(w, 20_000)                         # builds / warms the oracle library
         n_s, dt_s, cores, desc = oracle_step_sample(w, args.cpu_sample)
         cpu = dict(value=n_s / dt_s / 1e6, unit="Mparticle-steps/s", cores=cores, kind="oracle", sample=desc,
-                   seconds=dt_s)
+                   seconds=dt_s, mean_neighbours_of_sample=oracle_sample_neighbours(w, args.cpu_sample),
+                   mean_neighbours_of_workload=pairs / float(n))
 
     line = dict(
         metric=METRIC, value=value, unit="Mparticle-steps/s", n_gpus=world, steps=args.steps, warmup=args.warmup,
@@ -405,6 +477,8 @@ def main():
         data="synthetic",
         config=dict(workload=f"config{args.config}: 3-D dam break, {w.n_fluid} fluid + {n - w.n_fluid} boundary "
                              f"particles, {w.n_slabs} logical x-slabs",
+                    state=(f"disordered: scrambled start + {args.disorder} steps before warm-up" if args.disorder
+                           else "rest-state lattice with seeded jitter (BASELINE configs)"),
                     n_particles=n, n_slabs=w.n_slabs, cells=int(v.ncells), cell_bits=int(v.cell_bits),
                     radix_passes=passes, dt=("variable, cfl 0.2" if args.adaptive else w.dt), multi_gpu="replicas only",
                     l2="no flush: per-step working set %.1f GB >> 126 MB L2" % (n * 198e-9)

@@ -5,11 +5,19 @@
 // Tait equation of state L112, dynamic boundary particles L116.
 //
 // Design ("a7"):
-//  * A CTA owns a tile of 2 x 2 cell columns x zb cells.  The candidates of all its targets lie in the
-//    4 x 4 columns x (zb + 2) cells around it: with z-fastest keys that is 16 contiguous ranges of the
-//    sorted arrays, fetched into shared memory by 32 bulk asynchronous copies (cp.async.bulk, the 1-D
-//    TMA path) that complete on an mbarrier; a conversion pass turns the raw records in place into
-//    tile-relative coordinates (origin = tile centre) and adds  m_j = |x_j|^2 - thr.
+//  * Work = the non-empty TILES of 2 x 2 cell columns x zb cells, listed by ia_tile_list_kernel.  The
+//    candidates of all targets of a tile lie in the 4 x 4 columns x (zb + 2) cells around it: with
+//    z-fastest keys that is 16 contiguous ranges of the sorted arrays.
+//  * interact_mma_kernel is PERSISTENT (one CTA per SM) and warp-specialised.  The first IM_NP warps are the
+//    producers (one group, named barrier): they take the next tile from the list (atomic counter), read its piece of the cell table, fetch
+//    the 16 ranges into one of two shared-memory stages with 32 bulk asynchronous copies
+//    (cp.async.bulk, the 1-D TMA path, completing on an mbarrier), convert the raw records in place
+//    into tile-relative coordinates (origin = tile centre) + m_j = |x_j|^2 - thr, order the tile's
+//    targets and publish the stage on a "full" mbarrier.  The other warps are consumers: each takes
+//    chunks of 32 targets of a published stage from a shared counter, filters and drains them (below),
+//    writes their rates and, when a stage has no chunk left, releases it on an "empty" mbarrier and
+//    moves on to the other stage.  Staging of tile k + 1 therefore runs under the arithmetic of tile k,
+//    and there is no CTA-wide barrier anywhere after the set-up.
 //  * FILTER (warp-cooperative, on the tensor cores).  The distance test IS a dense contraction:
 //        D_ij = |x_i|^2 + m_j - 2 x_i . x_j  =  r_ij^2 - thr        (K = 4: x, y, z, 1 | m)
 //    One mma.sync m16n8k4 (tf32 inputs, fp32 accumulate; the |x_i|^2 term rides in the accumulator
@@ -23,9 +31,12 @@
 //  * DRAIN (one lane = one target).  Lanes pop their hits in ascending candidate order and evaluate the
 //    pair term in fp32, two pairs per instruction with the packed FFMA2/FMUL2/FADD2 forms of sm_100a
 //    (fma.rn.f32x2): the kernel is bound by instruction issue, not by the FP32 pipes.  Hits are consumed
-//    in groups of four; an incomplete group is carried over to the next round of the mask ring, so the
-//    summation order of a target depends only on its own hit sequence (per-sub-domain execution
-//    reproduces the global pass bit for bit, slab_exec.cu).
+//    in groups of four; the k-th hit of a target always lands in sub-lane k & 1, so the summation order
+//    of a target depends only on its own hit sequence (per-sub-domain execution reproduces the global
+//    pass bit for bit, slab_exec.cu).
+//  * Tiles with more candidates than a stage holds, or more targets than its target list, are split into
+//    several ITEMS (target range x candidate batch); the items of a batch after the first ADD to the
+//    rates already written (the producer publishes them only after the previous item has drained).
 //  * No tensor cores in the pair term: it is not a contraction.
 //
 // FP32-ALU bound ("bound": "alu" in bench.py).
@@ -34,52 +45,71 @@
 
 namespace sph {
 
-#ifndef SPH_IM_THREADS
-#define SPH_IM_THREADS 352
+#ifndef SPH_IM_CONSUMERS
+#define SPH_IM_CONSUMERS 12
+#endif
+#ifndef SPH_IM_PRODUCERS
+#define SPH_IM_PRODUCERS 4
 #endif
 #ifndef SPH_IM_RB
 #define SPH_IM_RB 9
 #endif
-#ifndef SPH_IM_MINBLOCKS
-#define SPH_IM_MINBLOCKS 2
-#endif
-constexpr int IM_THREADS = SPH_IM_THREADS;   // 11 warps: 2 x 2 x 3 cells x 27 particles = 324 targets
-constexpr int IM_WARPS = IM_THREADS / 32;
+constexpr int IM_NC = SPH_IM_CONSUMERS;      // consumer warps
+constexpr int IM_NP = SPH_IM_PRODUCERS;       // producer warps
+constexpr int IM_THREADS = 32 * (IM_NC + IM_NP);
+constexpr int IM_MAXT = 352;                 // targets per item: 2 x 2 x 3 cells x 27 particles = 324
 constexpr int IM_COLS = 16;                  // staged columns: 4 x 4
 constexpr int IM_ZMAX = 6;                   // max cells per z-block (tf32 model: |z| <= (zb + 2) h)
 constexpr int IM_CAP = 2304;                 // staged record slots per batch = 36 blocks of 64
 constexpr int IM_BATCH = IM_CAP - 128;       // particles per batch (16 x 5 x 27 = 2160): the 4 x-rows start at multiples
                                              // of 32 slots, which costs up to 4 x 31 padding slots
 constexpr int IM_RB = SPH_IM_RB;             // mask ring: blocks of 64 candidates per warp per round
+constexpr int IM_STAGES = 2;
 constexpr float IM_WIDE_N = -3.0e38f;        // |x|^2 stand-in of "wide" tiles: every real record is a hit
 constexpr float IM_FAR = 1e15f;              // coordinate of the dummy partner: r2 = 3e30 is finite, shape = 0
 constexpr float IM_TINY = 1e-30f;            // added to r2: a coincident pair (the particle itself) adds exactly 0
+constexpr uint32_t IM_CTR_NTILES = 16, IM_CTR_NEXT = 17;    // words of sph_ctx::counters
 static_assert(IM_CAP % 64 == 0 && IM_RB >= 2, "blocks of 64; the ring doubles as scratch for the A rows");
+static_assert(IM_MAXT % 32 == 0, "chunks of 32 targets");
 
-struct __align__(1024) ImSmem {
+struct __align__(1024) ImStage {    // recA at a multiple of 1024 B: the slot swizzle is applied to shared ADDRESSES
     float4 recA[IM_CAP + 1];                 // x, y, z relative to the tile centre, p/rho^2; slot IM_CAP = dummy partner
     float4 recB[IM_CAP + 1];                 // vx, vy, vz, rho/rho0 (sign = boundary type if masses differ)
     float marr[IM_CAP + 4];                  // m_j = |x_j|^2 - thr, rounded to tf32
-    uint32_t mask[IM_WARPS][IM_RB][64];      // per warp and ring slot: [half][target lane] hit masks of 32 candidates
+    uint32_t tglob[IM_MAXT];                 // targets of the item, ordered by (x-row, position inside the cell along x):
+                                             // global index | own column << 28
+    uint32_t row_astart[5];                  // slot of the first record of each staged x-row (multiple of 32); [4] = end
+    uint32_t ntargets;
+    uint32_t chunk_ctr;                      // next chunk of 32 targets
+    uint32_t wide;                           // some record lies outside the tf32 error model
+    uint32_t accumulate;                     // add to the rates already in memory (second and later batches)
+    uint32_t exit;                           // no more work
+    float ox, oy, oz, bxy, bzz;              // tile origin and the bounds of the tf32 error model
+};
+
+struct __align__(1024) ImSmem {
+    ImStage st[IM_STAGES];
+    uint32_t mask[IM_NC][IM_RB][64];         // per consumer warp and ring slot: [half][target lane] hit masks of 32 candidates
+    // producer-private
     uint32_t cbt[IM_COLS][IM_ZMAX + 3];      // cell_begin of the 16 columns over [zlo, zhi]
     uint32_t col_vstart[IM_COLS + 1];        // virtual start of each column in the concatenation
-    uint32_t stage_lo[IM_COLS], stage_hi[IM_COLS];   // global index range of the column staged in this batch
-    int32_t stage_off[IM_COLS];              // arrival index = global index + stage_off
-    uint32_t row_astart[5];                  // slot of the first record of each staged x-row (multiple of 32); [4] = end
-    uint32_t row_len[4];                     // records of the row in this batch
-    uint32_t tbase[4], tcount[4], tstart[5]; // target ranges of the 2 x 2 own columns
-    uint32_t bcnt[32];                       // target sort: bucket counts, then bucket starts
-    uint32_t perm[IM_THREADS];               // target sort: (global index | own column << 28) by sorted position
-    unsigned long long mbar;                 // completion barrier of the bulk copies
-    uint32_t wide;                           // some particle lies outside the tf32 error model
+    uint32_t tstart[5], tbase[4], tcnt[4];   // target ranges of the 2 x 2 own columns
+    uint32_t bcnt[32];                       // target ordering: bucket counts, then bucket starts
+    uint32_t tkey[IM_MAXT];                  // target ordering: bucket | rank << 8 | own column << 28
+    uint32_t tidx[IM_MAXT];                  // target ordering: global index
+    uint32_t row_len[4];
+    uint32_t tile;                           // the tile the producers work on
+    unsigned long long full[IM_STAGES], empty[IM_STAGES], tma;
 };
 
 struct ImArgs {
     int zb, nzb;                             // cells per z-block, z-blocks per column
-    int tx0, nty;                            // first x tile, tiles along y
+    int tx0, nty, ntx;                       // first x tile, tiles along y and x
     int cx_first, cx_end;                    // cell planes that hold the targets
     int cand_lo, cand_hi;                    // cell planes that exist in the arrays (per-slab execution), inclusive
     float thr2;                              // filter threshold, physical units
+    const uint32_t *tile_list;               // non-empty tiles (ia_tile_list_kernel)
+    uint32_t *ctr;                           // [IM_CTR_NTILES] = tiles listed, [IM_CTR_NEXT] = next tile to hand out
 };
 
 // ---- packed fp32 pairs (sm_100a FFMA2 / FMUL2 / FADD2) --------------------------------------------
@@ -133,7 +163,10 @@ __device__ __forceinline__ void im_sts_u16(uint32_t addr, uint32_t v)
 __device__ __forceinline__ void mbar_init(uint32_t mbar, uint32_t count)
 {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(mbar), "r"(count) : "memory");
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t mbar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(mbar) : "memory");
 }
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t mbar, uint32_t bytes)
 {
@@ -143,8 +176,9 @@ __device__ __forceinline__ void mbar_wait(uint32_t mbar, uint32_t parity)
 {
     uint32_t done;
     do {
-        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-                     : "=r"(done) : "r"(mbar), "r"(parity) : "memory");
+        // the thread sleeps until the phase completes or the time hint (ns) runs out: no issue slots are spent polling
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(done) : "r"(mbar), "r"(parity), "r"(20000u) : "memory");
     } while (!done);
 }
 // 1-D bulk asynchronous copy global -> shared (SASS: UBLKCP); bytes % 16 == 0, both sides 16-byte aligned
@@ -194,11 +228,514 @@ __device__ __forceinline__ float kernel_shape(float r, float rinv, const PhysC &
     }
 }
 
-int interact_mma_threads() { return IM_THREADS; }
+int interact_mma_targets() { return IM_MAXT; }
 int interact_mma_zmax() { return IM_ZMAX; }
 
+__device__ __forceinline__ void im_tile_coords(uint32_t b, const ImArgs &A, int &cx0, int &cy0, int &cz0)
+{
+    cz0 = (int)(b % (uint32_t)A.nzb) * A.zb;
+    b /= (uint32_t)A.nzb;
+    cy0 = (int)(b % (uint32_t)A.nty) * 2;
+    cx0 = ((int)(b / (uint32_t)A.nty) + A.tx0) * 2;
+}
+
+// ---- list of the non-empty tiles (most of a dam-break tank holds no particle) ------------------------
+__global__ void __launch_bounds__(256)
+ia_tile_list_kernel(const uint32_t *__restrict__ cell_begin, GridC g, ImArgs A, uint32_t ntiles, uint32_t *list)
+{
+    const uint32_t b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= ntiles) return;
+    int cx0, cy0, cz0;
+    im_tile_coords(b, A, cx0, cy0, cz0);
+    const int cz1 = min(cz0 + A.zb, g.nc[2]);
+    uint32_t any = 0;
+#pragma unroll
+    for (int t = 0; t < 4; ++t) {
+        const int x = cx0 + (t >> 1), y = cy0 + (t & 1);
+        if (x >= A.cx_first && x < A.cx_end && y < g.nc[1]) {
+            const uint32_t colbase = (uint32_t)(x * g.nc[1] + y) * g.nc[2];
+            any |= cell_begin[colbase + cz1] - cell_begin[colbase + cz0];
+        }
+    }
+    if (any) list[atomicAdd(A.ctr + IM_CTR_NTILES, 1u)] = b;     // any order: a tile's result does not depend on it
+}
+
+// ---- producers: IM_NP warps working as one group (named barrier 1) -----------------------------------
+__device__ __forceinline__ void im_pbar()
+{
+    asm volatile("bar.sync 1, %0;" ::"n"(32 * IM_NP) : "memory");
+}
+
+template <bool UNIFORM>
+__device__ __forceinline__ void im_produce(ImSmem &S, const float4 *__restrict__ pos4, const float4 *__restrict__ velrho4,
+                                           const uint32_t *__restrict__ idt, const uint32_t *__restrict__ cell_begin,
+                                           const GridC &g, const PhysC &ph, const ImArgs &A)
+{
+    const int ptid = threadIdx.x, lane = ptid & 31, pwarp = ptid >> 5;
+    constexpr int PT = 32 * IM_NP;
+    const uint32_t full_mask = 0xffffffffu;
+    const uint32_t tma = (uint32_t)__cvta_generic_to_shared(&S.tma);
+    const uint32_t ntiles = A.ctr[IM_CTR_NTILES];
+    const float cell = 2.0f * ph.h;
+    uint32_t it = 0, tma_phase = 0;
+
+    while (true) {
+        im_pbar();                                                   // the previous tile's tables are no longer read
+        if (ptid == 0) S.tile = atomicAdd(A.ctr + IM_CTR_NEXT, 1u);
+        im_pbar();
+        uint32_t b = S.tile;
+        if (b >= ntiles) break;
+        b = A.tile_list[b];
+        int cx0, cy0, cz0;
+        im_tile_coords(b, A, cx0, cy0, cz0);
+        const int cz1 = min(cz0 + A.zb, g.nc[2]);
+        const int zlo = max(cz0 - 1, 0), zhi = min(cz1 + 1, g.nc[2]);
+        const int nz = zhi - zlo;                                    // <= zb + 2
+
+        // ---- the tile's piece of the cell table
+        if (ptid < 4) {
+            const int x = cx0 + (ptid >> 1), y = cy0 + (ptid & 1);
+            uint32_t tb = 0, te = 0;
+            if (x >= A.cx_first && x < A.cx_end && y < g.nc[1]) {
+                const uint32_t colbase = (uint32_t)(x * g.nc[1] + y) * g.nc[2];
+                tb = cell_begin[colbase + cz0];
+                te = cell_begin[colbase + cz1];
+            }
+            S.tbase[ptid] = tb;
+            S.tcnt[ptid] = te - tb;
+        }
+        for (int k = ptid; k < IM_COLS * (nz + 1); k += PT) {
+            const int col = k / (nz + 1), z = k % (nz + 1);
+            const int x = cx0 - 1 + (col >> 2), y = cy0 - 1 + (col & 3);
+            uint32_t v = 0;
+            if (x >= A.cand_lo && x <= A.cand_hi && y >= 0 && y < g.nc[1])
+                v = cell_begin[(uint32_t)(x * g.nc[1] + y) * g.nc[2] + zlo + z];
+            S.cbt[col][z] = v;                   // columns that do not exist: all 0 => empty ranges
+        }
+        im_pbar();
+        if (pwarp == 0) {
+            const uint32_t len = lane < IM_COLS ? S.cbt[lane][nz] - S.cbt[lane][0] : 0u;
+            const uint32_t tcount = lane < 4 ? S.tcnt[lane] : 0u;
+            uint32_t inc = len, tinc = tcount;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t t = __shfl_up_sync(full_mask, inc, o), u = __shfl_up_sync(full_mask, tinc, o);
+                if (lane >= o) { inc += t; tinc += u; }
+            }
+            if (lane <= IM_COLS) S.col_vstart[lane] = inc - len;     // lane 16: the total
+            if (lane <= 4) S.tstart[lane] = tinc - tcount;           // lane 4: the total
+        }
+        im_pbar();
+        const uint32_t total = S.col_vstart[IM_COLS];
+        const uint32_t ttotal = S.tstart[4];
+
+        // tile-relative coordinates: origin = centre of the staged region.  |x|, |y| <= 4h and |z| <= nz h for
+        // every particle that lies inside its cell - the range the tf32 error model (filter_thr) assumes; a
+        // particle outside it (it left the grid and sits clamped in an edge cell, reading A13) switches the
+        // filter off ("wide": every candidate passes, the drain decides).
+        const float ox = fmaf((float)(cx0 + 1), cell, g.min[0]);
+        const float oy = fmaf((float)(cy0 + 1), cell, g.min[1]);
+        const float oz = fmaf((float)zlo + 0.5f * (float)nz, cell, g.min[2]);
+        const float bxy = 2.0f * cell * 1.002f, bzz = 0.5f * (float)nz * cell * 1.002f;
+
+        for (uint32_t t0 = 0; t0 < ttotal; t0 += IM_MAXT) {
+            const uint32_t nT = min((uint32_t)IM_MAXT, ttotal - t0);
+            for (uint32_t bstart = 0; bstart < total; bstart += IM_BATCH) {
+                const uint32_t bend = min(total, bstart + IM_BATCH);
+                const uint32_t s = it & 1u, use = it >> 1;
+                ImStage &T = S.st[s];
+                mbar_wait((uint32_t)__cvta_generic_to_shared(&S.empty[s]), (use & 1u) ^ 1u);
+                // a later batch adds to what the previous item wrote: wait until that item has drained
+                if (bstart > 0) mbar_wait((uint32_t)__cvta_generic_to_shared(&S.empty[s ^ 1u]), ((it - 1u) >> 1) & 1u);
+                const uint32_t recA_addr = (uint32_t)__cvta_generic_to_shared(T.recA);
+                const uint32_t recB_addr = (uint32_t)__cvta_generic_to_shared(T.recB);
+
+                // ---- slots of this batch: x-row r starts at a multiple of 32 (a target's window of three rows
+                // is then a whole number of 32-candidate mask words)
+                if (ptid == 0) {
+                    uint32_t a = 0;
+                    for (int r = 0; r < 4; ++r) {
+                        const uint32_t lo = min(max(S.col_vstart[4 * r], bstart), bend);
+                        const uint32_t hi = min(max(S.col_vstart[4 * r + 4], bstart), bend);
+                        T.row_astart[r] = a;
+                        S.row_len[r] = hi - lo;
+                        a = (a + (hi - lo) + 31u) & ~31u;
+                    }
+                    T.row_astart[4] = a;
+                    T.ntargets = nT;
+                    T.chunk_ctr = 0u;
+                    T.wide = 0u;
+                    T.accumulate = bstart > 0 ? 1u : 0u;
+                    T.exit = 0u;
+                    T.ox = ox; T.oy = oy; T.oz = oz; T.bxy = bxy; T.bzz = bzz;
+                    mbar_arrive_expect_tx(tma, (bend - bstart) * 32u);
+                }
+                if (ptid < 32) S.bcnt[ptid] = 0u;
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");    // generic writes of the last use < bulk copies
+                im_pbar();
+                // ---- stage: one bulk copy per column and array, all completing on the mbarrier
+                if (ptid < IM_COLS) {
+                    const int r = ptid >> 2;
+                    const uint32_t vs = S.col_vstart[ptid], ve = S.col_vstart[ptid + 1];
+                    const uint32_t lo = max(vs, bstart), hi = min(ve, bend);
+                    const uint32_t rlo = min(max(S.col_vstart[4 * r], bstart), bend);    // first particle of the row in the batch
+                    if (lo < hi) {
+                        const uint32_t gl = S.cbt[ptid][0] + (lo - vs);
+                        const uint32_t a = T.row_astart[r] + (lo - rlo);
+                        bulk_g2s(recA_addr + 16u * a, pos4 + gl, 16u * (hi - lo), tma);
+                        bulk_g2s(recB_addr + 16u * a, velrho4 + gl, 16u * (hi - lo), tma);
+                    }
+                }
+                // ---- meanwhile: order the targets by (x-row, position inside the cell along x).  How many hits
+                // a target meets in each x-row of the staged region depends on where it sits in its cell along
+                // x; the drain works row by row, so a warp whose lanes share that position keeps all its lanes
+                // busy in every row.  The order of a target's own sum does not depend on its lane.
+                for (uint32_t q = ptid; q < nT; q += PT) {
+                    const uint32_t tq = t0 + q;
+                    int tc = 0;
+#pragma unroll
+                    for (int t = 1; t < 4; ++t) tc += (tq >= S.tstart[t]) ? 1 : 0;
+                    const uint32_t i = S.tbase[tc] + (tq - S.tstart[tc]);
+                    const float px = __ldg(reinterpret_cast<const float *>(pos4 + i)) - ox;    // column tc >> 1 spans
+                    const float ph16 = (px - (float)((tc >> 1) - 1) * cell) * (16.0f / cell);     // [(tx-1) cell, tx cell)
+                    const uint32_t bk = (uint32_t)(tc >> 1) * 16u + (uint32_t)min(max(__float2int_rd(ph16), 0), 15);
+                    const uint32_t rk = atomicAdd(&S.bcnt[bk], 1u);
+                    S.tkey[q] = bk | (rk << 8) | ((uint32_t)tc << 28);
+                    S.tidx[q] = i;
+                }
+                im_pbar();
+                if (pwarp == 0) {
+                    const uint32_t v = S.bcnt[lane];
+                    uint32_t inc = v;
+#pragma unroll
+                    for (int o = 1; o < 32; o <<= 1) {
+                        const uint32_t t = __shfl_up_sync(full_mask, inc, o);
+                        if (lane >= o) inc += t;
+                    }
+                    S.bcnt[lane] = inc - v;
+                }
+                im_pbar();
+                for (uint32_t q = ptid; q < nT; q += PT) {
+                    const uint32_t k = S.tkey[q];
+                    T.tglob[S.bcnt[k & 31u] + ((k >> 8) & 0xFFFFFu)] = S.tidx[q] | (k & 0x30000000u);
+                }
+                mbar_wait(tma, tma_phase);
+                tma_phase ^= 1u;
+                // ---- convert in place: tile-relative coordinates, m = |x|^2 - thr (tf32), rho -> rho/rho0; the
+                // padding slots between the rows and up to the next block of 64 become records that never hit
+                const uint32_t aend = T.row_astart[4];
+                const uint32_t nconv = (aend + 63u) & ~63u;
+                uint32_t wide = 0u;
+                for (uint32_t a0 = 64u * (uint32_t)pwarp; a0 < nconv; a0 += 64u * IM_NP) {
+                    float4 ra[2], rb[2];
+                    float m[2];
+#pragma unroll
+                    for (int u = 0; u < 2; ++u) {
+                        const uint32_t a = a0 + 32u * u + lane;
+                        int r = 0;
+#pragma unroll
+                        for (int q = 1; q < 4; ++q) r += (a >= T.row_astart[q]) ? 1 : 0;
+                        const uint32_t k = a - T.row_astart[r];
+                        ra[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+                        rb[u] = make_float4(0.f, 0.f, 0.f, 1.f);
+                        m[u] = __int_as_float(0x7f800000);                        // +inf: D > 0 against any target
+                        if (a < aend && k < S.row_len[r]) {
+                            ra[u] = T.recA[a];
+                            rb[u] = T.recB[a];
+                            ra[u].x -= ox; ra[u].y -= oy; ra[u].z -= oz;
+                            if (!(fabsf(ra[u].x) <= bxy && fabsf(ra[u].y) <= bxy && fabsf(ra[u].z) <= bzz)) wide = 1u;
+                            m[u] = tf32_rna(fmaf(ra[u].z, ra[u].z, fmaf(ra[u].y, ra[u].y, ra[u].x * ra[u].x)) - A.thr2);
+                            rb[u].w *= ph.inv_rho0;
+                            if (!UNIFORM) {
+                                const uint32_t vv = min(max(S.col_vstart[4 * r], bstart), bend) + k;   // index in the concatenation
+                                int col = 0;
+#pragma unroll
+                                for (int q = 1; q < IM_COLS; ++q) col += (vv >= S.col_vstart[q]) ? 1 : 0;
+                                const uint32_t j = S.cbt[col][0] + (vv - S.col_vstart[col]);
+                                if (__ldg(idt + j) & TYPE_BIT) rb[u].w = -rb[u].w;
+                            }
+                        }
+                    }
+                    __syncwarp();                                // the 32 lanes cover aligned runs of 32 slots
+#pragma unroll
+                    for (int u = 0; u < 2; ++u) {
+                        const uint32_t a = a0 + 32u * u + lane;
+                        const uint32_t sw = a ^ ((a >> 3) & 6u);     // swizzle: the 8 records of an mma B fragment (slots
+                        T.recA[sw] = ra[u];                          // 2j + c + 16 q') fall on 8 different 16-byte bank groups
+                        T.recB[sw] = rb[u];
+                        T.marr[sw] = m[u];
+                    }
+                }
+                if (__any_sync(full_mask, wide != 0u) && lane == 0) T.wide = 1u;
+                im_pbar();
+                if (ptid == 0) mbar_arrive((uint32_t)__cvta_generic_to_shared(&S.full[s]));
+                ++it;
+            }
+        }
+    }
+    // ---- no more work
+    {
+        const uint32_t s = it & 1u, use = it >> 1;
+        mbar_wait((uint32_t)__cvta_generic_to_shared(&S.empty[s]), (use & 1u) ^ 1u);
+        if (ptid == 0) {
+            S.st[s].exit = 1u;
+            mbar_arrive((uint32_t)__cvta_generic_to_shared(&S.full[s]));
+        }
+    }
+}
+
+// ---- consumer: one chunk of 32 targets against the stage --------------------------------------------
 template <int KERNEL, bool UNIFORM, bool GAMMA7, bool MU>
-__global__ void __launch_bounds__(IM_THREADS, SPH_IM_MINBLOCKS)
+__device__ __forceinline__ void im_chunk(ImStage &T, uint32_t mwarp, uint32_t chunk,
+                                         const float4 *__restrict__ pos4, const float4 *__restrict__ velrho4,
+                                         const uint32_t *__restrict__ idt, float4 *__restrict__ acc4,
+                                         float *__restrict__ mu_out, const PhysC &ph)
+{
+    const int lane = threadIdx.x & 31;
+    const uint32_t full_mask = 0xffffffffu;
+    const int g8 = lane >> 2, qd = lane & 3;
+    const uint32_t recA_addr = (uint32_t)__cvta_generic_to_shared(T.recA);
+    const uint32_t recB_addr = (uint32_t)__cvta_generic_to_shared(T.recB);
+    const uint32_t marr_addr = (uint32_t)__cvta_generic_to_shared(T.marr);
+    const uint32_t ab_delta = recB_addr - recA_addr;
+    const uint32_t dummy_addr = recA_addr + 16u * (uint32_t)IM_CAP;
+
+    // constants of the pair term (the packed instructions take a scalar operand for both lanes)
+    const float kvisc = -ph.alpha_h * ph.c0 * ph.inv_rho0;       // Pi_ij = kvisc * poly * min(v.r, 0) / (r2 + eta2)
+    const f2 c_tiny = pk(IM_TINY, IM_TINY), c_eta2 = pk(ph.eta2, ph.eta2);
+    const f2 c_mih = pk(-ph.inv_h_half, -ph.inv_h_half), c_one = pk(1.0f, 1.0f), c_kv = pk(kvisc, kvisc);
+    const float cexp = 0.5f * (float)(ph.gamma - 1);
+
+    const uint32_t tq = chunk * 32u + (uint32_t)lane;
+    const bool active = tq < T.ntargets;
+    const uint32_t pe = active ? T.tglob[tq] : 0u;
+    const uint32_t i = pe & 0x0FFFFFFFu;
+    const int tx = (int)(pe >> 29);
+    float4 pi = make_float4(T.ox, T.oy, T.oz, 0.f), vi = make_float4(0.f, 0.f, 0.f, ph.rho0);
+    bool fluid = false;
+    if (active) {
+        pi = pos4[i];
+        vi = velrho4[i];
+        fluid = (idt[i] & TYPE_BIT) == 0;
+    }
+    const float xi = pi.x - T.ox, yi = pi.y - T.oy, zi = pi.z - T.oz;
+    const bool out = active && !(fabsf(xi) <= T.bxy && fabsf(yi) <= T.bxy && fabsf(zi) <= T.bzz);
+    const bool wide = __any_sync(full_mask, out) || T.wide != 0u;
+    const float ui = vi.w * ph.inv_rho0;
+    const float ui2 = GAMMA7 ? ui * ui : __powf(ui, cexp);   // gamma = 7: u^2; else u^((gamma-1)/2)
+    // x-rows of the staged region this warp's targets need: [txmin, txmax + 2]
+    const int txmin = __reduce_min_sync(full_mask, active ? tx : 2);
+    const int txmax = __reduce_max_sync(full_mask, active ? tx : -1);
+    // target side of the distance product
+    const float xh = tf32_rna(xi), yh = tf32_rna(yi), zh = tf32_rna(zi);
+    const float nn = fmaf(zh, zh, fmaf(yh, yh, xh * xh));
+
+    // fragment addressing: lanes 0..2 of a quad read x, y, z of the record, lane 3 reads m.
+    // mma group j of a block of 64 slots holds the slots 16 (n >> 1) + 2 j + (n & 1), n = 0..7, so that
+    // the 16 sign bits a lane collects for one target are 16 CONSECUTIVE slots of the target's mask.
+    const uint32_t sh = qd < 3 ? 4u : 2u;
+    const uint32_t lbase = (qd < 3 ? recA_addr + 4u * qd : marr_addr) + ((uint32_t)(16 * (g8 >> 1)) << sh);
+    uint32_t foff[4];                         // swizzled slot of group j (j + 4: 8 slots further)
+#pragma unroll
+    for (int j = 0; j < 4; ++j) foff[j] = (uint32_t)((2 * j + (g8 & 1)) ^ (2 * (g8 >> 1))) << sh;
+    // masks are stored bit-reversed (slot s of the block = bit 63 - s of the target's 64-bit word), so
+    // that "highest set bit first" (one FLO) walks the candidates in ascending order
+    const uint32_t piece_addr = (uint32_t)((qd >> 1) * 128 + ((qd & 1) ^ 1) * 2 + 4 * g8);
+
+    f2 ax2 = pk(0.f, 0.f), ay2 = ax2, az2 = ax2, dr2 = ax2;
+    float mumax = 0.f;
+    uint32_t odd = 0;                         // parity of the hits consumed so far: the next hit's sub-lane
+
+    // two pairs at once: candidates at the shared addresses sa (low lane) and sb (high lane) of recA
+    // against this lane's target
+    auto pair2 = [&](uint32_t sa, uint32_t sb) {
+        const float4 ra = im_lds_f4(sa), rb = im_lds_f4(sb);
+        float4 va = im_lds_f4(sa + ab_delta), vb = im_lds_f4(sb + ab_delta);
+        const f2 dx = pk(xi - ra.x, xi - rb.x), dy = pk(yi - ra.y, yi - rb.y), dz = pk(zi - ra.z, zi - rb.z);
+        const f2 r2 = add2(fma2(dz, dz, fma2(dy, dy, mul2(dx, dx))), c_tiny);
+        float r2a, r2b;
+        upk(r2, r2a, r2b);
+        const float ia = rsqrt_fast(r2a), ib = rsqrt_fast(r2b);
+        float ma = 1.0f, mb = 1.0f;
+        if (!UNIFORM) {
+            ma = va.w < 0.f ? ph.mass_bound : ph.mass_fluid;
+            mb = vb.w < 0.f ? ph.mass_bound : ph.mass_fluid;
+            va.w = fabsf(va.w);
+            vb.w = fabsf(vb.w);
+        }
+        f2 F;
+        if (KERNEL == 0) {
+            const f2 r = mul2(r2, pk(ia, ib));
+            f2 t = fma2(r, c_mih, c_one);
+            float ta, tb;
+            upk(t, ta, tb);
+            t = pk(fmaxf(ta, 0.0f), fmaxf(tb, 0.0f));
+            F = mul2(mul2(t, t), t);
+        } else {
+            F = pk(kernel_shape<KERNEL>(r2a * ia, ia, ph), kernel_shape<KERNEL>(r2b * ib, ib, ph));
+        }
+        if (!UNIFORM) F = mul2(F, pk(ma, mb));
+        const f2 dvx = pk(vi.x - va.x, vi.x - vb.x), dvy = pk(vi.y - va.y, vi.y - vb.y),
+                 dvz = pk(vi.z - va.z, vi.z - vb.z);
+        const f2 dot = fma2(dvz, dz, fma2(dvy, dy, mul2(dvx, dx)));
+        dr2 = fma2(F, dot, dr2);                                     // Eq. (7)
+        // L112 with c = c0 u^e, rho = rho0 u:  Pi = -alpha h c0/rho0 * (ui^e + uj^e)/(ui + uj) * min(v.r,0)/(r2+eta2);
+        // for gamma = 7 (e = 3) the quotient is ui^2 - ui uj + uj^2
+        f2 poly;
+        if (GAMMA7) {
+            poly = pk(fmaf(va.w, va.w - ui, ui2), fmaf(vb.w, vb.w - ui, ui2));
+        } else {
+            poly = pk(__fdividef(ui2 + __powf(va.w, cexp), ui + va.w), __fdividef(ui2 + __powf(vb.w, cexp), ui + vb.w));
+        }
+        float qa, qb;
+        upk(add2(r2, c_eta2), qa, qb);
+        const float rca = rcp_fast(qa), rcb = rcp_fast(qb);
+        float da, db;
+        upk(dot, da, db);
+        const f2 w = mul2(pk(fminf(da, 0.0f), fminf(db, 0.0f)), pk(rca, rcb));
+        if (MU) {
+            const float mua = ph.h * fabsf(da) * rca, mub = ph.h * fabsf(db) * rcb;
+            mumax = fmaxf(mumax, (r2a < ph.four_h2 && ma != 0.0f) ? mua : 0.0f);
+            mumax = fmaxf(mumax, (r2b < ph.four_h2 && mb != 0.0f) ? mub : 0.0f);
+        }
+        const f2 ps = pk(pi.w + ra.w, pi.w + rb.w);
+        const f2 coef = mul2(F, fma2(mul2(poly, w), c_kv, ps));      // Eq. (9) without its sign and constants
+        ax2 = fma2(coef, dx, ax2);
+        ay2 = fma2(coef, dy, ay2);
+        az2 = fma2(coef, dz, az2);
+    };
+
+    if (txmax >= 0) {
+        // ---- A rows of the distance product, handed to the lanes that hold them as mma fragments.
+        // "wide" tiles: D = m - 3e38 < 0 for every real record, +inf for the padding slots.
+        uint32_t af[4];
+        float nf[4];
+        {
+            const uint32_t scratch = mwarp;                      // the mask ring doubles as scratch
+            float4 row = make_float4(-2.0f * xh, -2.0f * yh, -2.0f * zh, nn);
+            if (wide) row = make_float4(0.f, 0.f, 0.f, IM_WIDE_N);
+            if (!active) row = make_float4(0.f, 0.f, 0.f, __int_as_float(0x7f800000));
+            asm volatile("st.shared.v4.f32 [%0], {%1,%2,%3,%4};" ::"r"(scratch + 16u * (uint32_t)lane), "f"(row.x), "f"(row.y),
+                         "f"(row.z), "f"(row.w) : "memory");
+            __syncwarp();
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const float4 r = im_lds_f4(scratch + 16u * (uint32_t)(g8 + 8 * k));
+                const float a = qd == 0 ? r.x : (qd == 1 ? r.y : (qd == 2 ? r.z : 1.0f));
+                af[k] = __float_as_uint(a);
+                nf[k] = r.w;
+            }
+            __syncwarp();
+        }
+        // ---- one round of the mask ring per x-row of the staged region (sub-rounds if a row is longer
+        // than the ring): all lanes of a warp meet about the same number of hits in a row, so the
+        // drain that follows each filter pass keeps them busy together
+        for (int r = txmin; r <= min(txmax + 2, 3); ++r) {
+            const uint32_t e0 = T.row_astart[r] >> 5, e1 = T.row_astart[r + 1] >> 5;     // mask words of the row
+            const uint32_t e_cnt = (active && r >= tx && r <= tx + 2) ? e1 - e0 : 0u;     // ... that are this lane's
+            for (uint32_t rb0 = e0 >> 1; rb0 < ((e1 + 1u) >> 1); rb0 += IM_RB) {
+                const uint32_t nb = min((uint32_t)IM_RB, ((e1 + 1u) >> 1) - rb0);
+                // ---- FILTER: nb blocks of 64 slots against the warp's 32 targets
+                for (uint32_t bi = 0; bi < nb; ++bi) {
+                    const uint32_t bb = lbase + (((rb0 + bi) * 64u) << sh);
+                    uint32_t p0 = 0, p1 = 0, p2 = 0, p3 = 0;
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) {
+                        const uint32_t bf = im_lds_u32(bb + foff[j & 3] + ((uint32_t)(8 * (j >> 2)) << sh));
+                        float d0, d1, d2, d3, d4, d5, d6, d7;
+                        mma_tf32_k4(d0, d1, d2, d3, af[0], af[1], bf, nf[0], nf[0], nf[1], nf[1]);
+                        mma_tf32_k4(d4, d5, d6, d7, af[2], af[3], bf, nf[2], nf[2], nf[3], nf[3]);
+                        p0 = push_sign(d1, push_sign(d0, p0));
+                        p1 = push_sign(d3, push_sign(d2, p1));
+                        p2 = push_sign(d5, push_sign(d4, p2));
+                        p3 = push_sign(d7, push_sign(d6, p3));
+                    }
+                    const uint32_t ma = mwarp + bi * 256u + piece_addr;
+                    im_sts_u16(ma, p0);
+                    im_sts_u16(ma + 32u, p1);
+                    im_sts_u16(ma + 64u, p2);
+                    im_sts_u16(ma + 96u, p3);
+                }
+                __syncwarp();
+                // ---- DRAIN.  Survey of this lane's mask words of the round: which are non-empty (nz,
+                // bit 31 - k = word k) and how many hits they hold; the number of rounds of four pairs
+                // is then known for the whole warp.
+                uint32_t nz = 0, tot = 0;
+                const uint32_t mlane = mwarp + 4u * (uint32_t)lane;          // word k of the round at mlane + 128 k
+                for (uint32_t k = 0; k < 2u * nb; ++k) {
+                    uint32_t w = im_lds_u32(mlane + 128u * k);
+                    if ((2u * rb0 + k) - e0 >= e_cnt) w = 0u;                  // another row, or not this lane's row
+                    tot += (uint32_t)__popc(w);
+                    nz |= w ? (0x80000000u >> k) : 0u;
+                }
+                // a lane whose hit count is odd so far leaves its last hit alone in the LOW sub-lane; the
+                // next hit then belongs in the HIGH one: start with the dummy partner in the low sub-lane.
+                // cur = remaining hits of the current word (bit 31 - t = slot t of the word);
+                // atop = shared address of recA[slot of bit 0 of cur] (bit hb is 16 hb bytes below it);
+                // nxtw / nxta = the next non-empty word and its atop, fetched when the current word was taken,
+                // so that no shared-memory load sits on the chain from one pop to the next
+                uint32_t cur = odd ? 1u : 0u;
+                uint32_t atop = dummy_addr;
+                const uint32_t steps = __reduce_max_sync(full_mask, tot ? (tot + odd + 3u) >> 2 : 0u);
+                odd = (odd + tot) & 1u;
+                const uint32_t atop0 = recA_addr + 16u * (rb0 * 64u + 32u * 31u + 31u);   // word k: atop0 - 512 (31 - k)
+                const uint32_t mtop = mlane + 128u * 31u;                                   // word k at mtop - 128 (31 - k)
+                uint32_t nxtw, nxta;
+                {
+                    const uint32_t kb = bfind(nz);                                      // highest bit = lowest word
+                    const uint32_t w = im_lds_u32(mtop - 128u * (kb & 31u));
+                    nxtw = nz ? w : 0u;
+                    nxta = atop0 - 512u * kb;
+                    nz &= ~(1u << (kb & 31u));
+                }
+                // branch-free: the word after next is read in any case (word 0 when none is left)
+                auto pop = [&]() -> uint32_t {
+                    const uint32_t kb = bfind(nz);
+                    const uint32_t w = im_lds_u32(mtop - 128u * (kb & 31u));
+                    const bool take = cur == 0u;
+                    cur = take ? nxtw : cur;
+                    atop = take ? nxta : atop;
+                    nxtw = take ? (nz ? w : 0u) : nxtw;
+                    nxta = take ? atop0 - 512u * kb : nxta;
+                    nz = take ? nz & ~(1u << (kb & 31u)) : nz;
+                    const uint32_t hb = bfind(cur);                                     // 0xFFFFFFFF if cur == 0
+                    const uint32_t lin = cur ? atop - 16u * hb : dummy_addr;
+                    cur &= ~(1u << (hb & 31u));
+                    return lin ^ ((lin >> 3) & 0x60u);                                  // slot swizzle, in bytes
+                };
+                // software pipeline: the addresses of step st + 1 are popped before the pairs of step st are evaluated
+                uint32_t sa = pop(), sb = pop(), sc = pop(), sd = pop();
+                for (uint32_t st = 0; st < steps; ++st) {
+                    const uint32_t na = pop(), nb2 = pop(), nc = pop(), nd = pop();     // past the last hit: dummy partners
+                    pair2(sa, sb);
+                    pair2(sc, sd);
+                    sa = na; sb = nb2; sc = nc; sd = nd;
+                }
+                __syncwarp();
+            }
+        }
+    }
+    if (active) {
+        float a0, a1, b0, b1, c0, c1, d0, d1;
+        upk(ax2, a0, a1); upk(ay2, b0, b1); upk(az2, c0, c1); upk(dr2, d0, d1);
+        const float k = UNIFORM ? ph.kF * ph.mass_fluid : ph.kF;
+        float ax = -k * (a0 + a1), ay = -k * (b0 + b1), az = -k * (c0 + c1);
+        float dr = k * (d0 + d1);
+        if (T.accumulate) {                      // a later batch of the tile's candidates
+            const float4 o = acc4[i];
+            ax += o.x; ay += o.y; az += o.z; dr += o.w;
+            if (MU) mumax = fmaxf(mumax, mu_out[i]);
+        } else if (fluid) {
+            ax += ph.g[0]; ay += ph.g[1]; az += ph.g[2];
+        }
+        if (!fluid) ax = ay = az = 0.f;
+        acc4[i] = make_float4(ax, ay, az, dr);
+        if (MU) mu_out[i] = mumax;
+    }
+}
+
+template <int KERNEL, bool UNIFORM, bool GAMMA7, bool MU>
+__global__ void __launch_bounds__(IM_THREADS, 1)
 interact_mma_kernel(const float4 *__restrict__ pos4, const float4 *__restrict__ velrho4,
                     const uint32_t *__restrict__ idt, const uint32_t *__restrict__ cell_begin,
                     float4 *__restrict__ acc4, float *__restrict__ mu_out, GridC g, PhysC ph, ImArgs A)
@@ -207,423 +744,38 @@ interact_mma_kernel(const float4 *__restrict__ pos4, const float4 *__restrict__ 
     ImSmem &S = *reinterpret_cast<ImSmem *>(im_raw);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
-    // ---- which tile
-    uint32_t b = blockIdx.x;
-    const int bz = b % A.nzb;
-    b /= A.nzb;
-    const int cy0 = (int)(b % A.nty) * 2;
-    const int cx0 = ((int)(b / A.nty) + A.tx0) * 2;
-    const int cz0 = bz * A.zb, cz1 = min(cz0 + A.zb, g.nc[2]);
-    const int zlo = max(cz0 - 1, 0), zhi = min(cz1 + 1, g.nc[2]);
-    const int nz = zhi - zlo;                                    // <= zb + 2
-    // ---- empty tiles (most of a dam-break tank) leave at once
-    {
-        uint32_t any = 0;
-#pragma unroll
-        for (int t = 0; t < 4; ++t) {
-            const int x = cx0 + (t >> 1), y = cy0 + (t & 1);
-            if (x >= A.cx_first && x < A.cx_end && y < g.nc[1]) {
-                const uint32_t colbase = (uint32_t)(x * g.nc[1] + y) * g.nc[2];
-                any |= cell_begin[colbase + cz1] - cell_begin[colbase + cz0];
-            }
-        }
-        if (any == 0) return;
-    }
-    const uint32_t mbar = (uint32_t)__cvta_generic_to_shared(&S.mbar);
     if (tid == 0) {
-        S.wide = 0u;
-        mbar_init(mbar, 1u);
-        S.recA[IM_CAP] = make_float4(IM_FAR, IM_FAR, IM_FAR, 0.f);
-        S.recB[IM_CAP] = make_float4(0.f, 0.f, 0.f, 1.f);
-    }
-    if (tid < 4) {
-        const int x = cx0 + (tid >> 1), y = cy0 + (tid & 1);
-        uint32_t tb = 0, te = 0;
-        if (x >= A.cx_first && x < A.cx_end && y < g.nc[1]) {
-            const uint32_t colbase = (uint32_t)(x * g.nc[1] + y) * g.nc[2];
-            tb = cell_begin[colbase + cz0];
-            te = cell_begin[colbase + cz1];
+        for (int s = 0; s < IM_STAGES; ++s) {
+            mbar_init((uint32_t)__cvta_generic_to_shared(&S.full[s]), 1u);
+            mbar_init((uint32_t)__cvta_generic_to_shared(&S.empty[s]), (uint32_t)IM_NC);
+            S.st[s].recA[IM_CAP] = make_float4(IM_FAR, IM_FAR, IM_FAR, 0.f);
+            S.st[s].recB[IM_CAP] = make_float4(0.f, 0.f, 0.f, 1.f);
         }
-        S.tbase[tid] = tb;
-        S.tcount[tid] = te - tb;
-    }
-    for (int k = tid; k < IM_COLS * (nz + 1); k += IM_THREADS) {
-        const int col = k / (nz + 1), z = k % (nz + 1);
-        const int x = cx0 - 1 + (col >> 2), y = cy0 - 1 + (col & 3);
-        uint32_t v = 0;
-        if (x >= A.cand_lo && x <= A.cand_hi && y >= 0 && y < g.nc[1])
-            v = cell_begin[(uint32_t)(x * g.nc[1] + y) * g.nc[2] + zlo + z];
-        S.cbt[col][z] = v;                   // columns that do not exist: all 0 => empty ranges
+        mbar_init((uint32_t)__cvta_generic_to_shared(&S.tma), 1u);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
-    if (tid == 0) {
-        uint32_t acc = 0;
-        for (int col = 0; col < IM_COLS; ++col) {
-            S.col_vstart[col] = acc;
-            acc += S.cbt[col][nz] - S.cbt[col][0];
-        }
-        S.col_vstart[IM_COLS] = acc;
-        acc = 0;
-        for (int t = 0; t < 4; ++t) { S.tstart[t] = acc; acc += S.tcount[t]; }
-        S.tstart[4] = acc;
+
+    if (warp < IM_NP) {
+        im_produce<UNIFORM>(S, pos4, velrho4, idt, cell_begin, g, ph, A);
+        return;
     }
-    __syncthreads();
-    const uint32_t total = S.col_vstart[IM_COLS];
-    const uint32_t ttotal = S.tstart[4];
-
-    // ---- tile-relative coordinates: origin = centre of the staged region.  |x|, |y| <= 4h and
-    // |z| <= nz h for every particle that lies inside its cell - the range the tf32 error model
-    // (filter_thr) assumes; a particle outside it (it left the grid and sits clamped in an edge cell,
-    // reading A13) switches the tile's filter off ("wide": every candidate passes, the drain decides).
-    const float cell = 2.0f * ph.h;
-    const float ox = fmaf((float)(cx0 + 1), cell, g.min[0]);
-    const float oy = fmaf((float)(cy0 + 1), cell, g.min[1]);
-    const float oz = fmaf((float)zlo + 0.5f * (float)nz, cell, g.min[2]);
-    const float bxy = 2.0f * cell * 1.002f, bzz = 0.5f * (float)nz * cell * 1.002f;
-
-    const uint32_t recA_addr = (uint32_t)__cvta_generic_to_shared(S.recA);
-    const uint32_t recB_addr = (uint32_t)__cvta_generic_to_shared(S.recB);
-    const uint32_t marr_addr = (uint32_t)__cvta_generic_to_shared(S.marr);
-    const uint32_t mwarp = (uint32_t)__cvta_generic_to_shared(&S.mask[warp][0][0]);
-    const uint32_t ab_delta = recB_addr - recA_addr;
-    const uint32_t dummy_addr = recA_addr + 16u * (uint32_t)IM_CAP;
-    const int g8 = lane >> 2, qd = lane & 3;
-    const uint32_t full_mask = 0xffffffffu;
-
-    // constants of the pair term (the packed instructions take a scalar operand for both lanes)
-    const float kvisc = -ph.alpha_h * ph.c0 * ph.inv_rho0;       // Pi_ij = kvisc * poly * min(v.r, 0) / (r2 + eta2)
-    const f2 c_tiny = pk(IM_TINY, IM_TINY), c_eta2 = pk(ph.eta2, ph.eta2);
-    const f2 c_mih = pk(-ph.inv_h_half, -ph.inv_h_half), c_one = pk(1.0f, 1.0f), c_kv = pk(kvisc, kvisc);
-    const float cexp = 0.5f * (float)(ph.gamma - 1);
-
-    uint32_t phase = 0;
-    for (uint32_t chunk = 0; chunk < ttotal; chunk += IM_THREADS) {
-        // ---- targets of this chunk, handed to the threads SORTED by (x-row, position inside the cell
-        // along x).  How many hits a target meets in each x-row of the staged region depends on where it
-        // sits in its cell along x; the drain works row by row, so a warp whose lanes share that position
-        // keeps all its lanes busy in every row (a lattice block at rest: 32 instead of 44 rounds of four
-        // pairs per target).  The order of a target's own sum does not depend on its lane.
-        const uint32_t nchunk = min((uint32_t)IM_THREADS, ttotal - chunk);
-        if (tid < 32) S.bcnt[tid] = 0u;
-        __syncthreads();
-        uint32_t my_i = 0, my_b = 0, my_r = 0, my_tcol = 0;
-        if ((uint32_t)tid < nchunk) {
-            const uint32_t tq = chunk + tid;
-            int tc = 0;
-#pragma unroll
-            for (int t = 1; t < 4; ++t) tc += (tq >= S.tstart[t]) ? 1 : 0;
-            my_tcol = (uint32_t)tc;
-            my_i = S.tbase[tc] + (tq - S.tstart[tc]);
-            const float px = __ldg(reinterpret_cast<const float *>(pos4 + my_i)) - ox;      // column tc >> 1 spans
-            const float ph16 = (px - (float)((tc >> 1) - 1) * cell) * (16.0f / cell);           // [(tx-1) cell, tx cell)
-            my_b = (uint32_t)(tc >> 1) * 16u + (uint32_t)min(max(__float2int_rd(ph16), 0), 15);
-            my_r = atomicAdd(&S.bcnt[my_b], 1u);
+    const uint32_t mwarp = (uint32_t)__cvta_generic_to_shared(&S.mask[warp - IM_NP][0][0]);
+    for (uint32_t it = 0;; ++it) {
+        const uint32_t s = it & 1u;
+        ImStage &T = S.st[s];
+        mbar_wait((uint32_t)__cvta_generic_to_shared(&S.full[s]), (it >> 1) & 1u);
+        if (T.exit) break;
+        const uint32_t nchunks = (T.ntargets + 31u) >> 5;
+        while (true) {
+            uint32_t c = 0;
+            if (lane == 0) c = atomicAdd(&T.chunk_ctr, 1u);
+            c = __shfl_sync(0xffffffffu, c, 0);
+            if (c >= nchunks) break;
+            im_chunk<KERNEL, UNIFORM, GAMMA7, MU>(T, mwarp, c, pos4, velrho4, idt, acc4, mu_out, ph);
         }
-        __syncthreads();
-        if (tid < 32) {                               // exclusive scan of the 32 bucket counts
-            const uint32_t v = S.bcnt[tid];
-            uint32_t inc = v;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const uint32_t t = __shfl_up_sync(full_mask, inc, o);
-                if (lane >= o) inc += t;
-            }
-            S.bcnt[tid] = inc - v;
-        }
-        __syncthreads();
-        if ((uint32_t)tid < nchunk) S.perm[S.bcnt[my_b] + my_r] = my_i | (my_tcol << 28);
-        __syncthreads();
-        const bool active = (uint32_t)tid < nchunk;
-        const uint32_t pe = active ? S.perm[tid] : 0u;
-        const uint32_t i = pe & 0x0FFFFFFFu;
-        const int tcol = (int)(pe >> 28);
-        const int tx = tcol >> 1;
-        float4 pi = make_float4(ox, oy, oz, 0.f), vi = make_float4(0.f, 0.f, 0.f, ph.rho0);
-        bool fluid = false;
-        if (active) {
-            pi = pos4[i];
-            vi = velrho4[i];
-            fluid = (idt[i] & TYPE_BIT) == 0;
-        }
-        const float xi = pi.x - ox, yi = pi.y - oy, zi = pi.z - oz;
-        if (active && !(fabsf(xi) <= bxy && fabsf(yi) <= bxy && fabsf(zi) <= bzz)) S.wide = 1u;
-        const float ui = vi.w * ph.inv_rho0;
-        const float ui2 = GAMMA7 ? ui * ui : __powf(ui, cexp);   // gamma = 7: u^2; else u^((gamma-1)/2)
-        // x-rows of the staged region this warp's targets need: [txmin, txmax + 2]
-        const int txmin = __reduce_min_sync(full_mask, active ? tx : 2);
-        const int txmax = __reduce_max_sync(full_mask, active ? tx : -1);
-        const bool warp_has = txmax >= 0;
-        // target side of the distance product
-        const float xh = tf32_rna(xi), yh = tf32_rna(yi), zh = tf32_rna(zi);
-        const float nn = fmaf(zh, zh, fmaf(yh, yh, xh * xh));
-
-        // fragment addressing: lanes 0..2 of a quad read x, y, z of the record, lane 3 reads m.
-        // mma group j of a block of 64 slots holds the slots 16 (n >> 1) + 2 j + (n & 1), n = 0..7, so that
-        // the 16 sign bits a lane collects for one target are 16 CONSECUTIVE slots of the target's mask.
-        const uint32_t sh = qd < 3 ? 4u : 2u;
-        const uint32_t lbase = (qd < 3 ? recA_addr + 4u * qd : marr_addr) + ((uint32_t)(16 * (g8 >> 1)) << sh);
-        uint32_t foff[4];                         // swizzled slot of group j (j + 4: 8 slots further)
-#pragma unroll
-        for (int j = 0; j < 4; ++j) foff[j] = (uint32_t)((2 * j + (g8 & 1)) ^ (2 * (g8 >> 1))) << sh;
-        // masks are stored bit-reversed (slot s of the block = bit 63 - s of the target's 64-bit word), so
-        // that "highest set bit first" (one FLO) walks the candidates in ascending order
-        const uint32_t piece_addr = (uint32_t)((qd >> 1) * 128 + ((qd & 1) ^ 1) * 2 + 4 * g8);
-
-        f2 ax2 = pk(0.f, 0.f), ay2 = ax2, az2 = ax2, dr2 = ax2;
-        float mumax = 0.f;
-        uint32_t odd = 0;                         // parity of the hits consumed so far: the next hit's sub-lane
-
-        // two pairs at once: candidates at the shared addresses sa (low lane) and sb (high lane) of recA
-        // against this lane's target
-        auto pair2 = [&](uint32_t sa, uint32_t sb) {
-            const float4 ra = im_lds_f4(sa), rb = im_lds_f4(sb);
-            float4 va = im_lds_f4(sa + ab_delta), vb = im_lds_f4(sb + ab_delta);
-            const f2 dx = pk(xi - ra.x, xi - rb.x), dy = pk(yi - ra.y, yi - rb.y), dz = pk(zi - ra.z, zi - rb.z);
-            const f2 r2 = add2(fma2(dz, dz, fma2(dy, dy, mul2(dx, dx))), c_tiny);
-            float r2a, r2b;
-            upk(r2, r2a, r2b);
-            const float ia = rsqrt_fast(r2a), ib = rsqrt_fast(r2b);
-            float ma = 1.0f, mb = 1.0f;
-            if (!UNIFORM) {
-                ma = va.w < 0.f ? ph.mass_bound : ph.mass_fluid;
-                mb = vb.w < 0.f ? ph.mass_bound : ph.mass_fluid;
-                va.w = fabsf(va.w);
-                vb.w = fabsf(vb.w);
-            }
-            f2 F;
-            if (KERNEL == 0) {
-                const f2 r = mul2(r2, pk(ia, ib));
-                f2 t = fma2(r, c_mih, c_one);
-                float ta, tb;
-                upk(t, ta, tb);
-                t = pk(fmaxf(ta, 0.0f), fmaxf(tb, 0.0f));
-                F = mul2(mul2(t, t), t);
-            } else {
-                F = pk(kernel_shape<KERNEL>(r2a * ia, ia, ph), kernel_shape<KERNEL>(r2b * ib, ib, ph));
-            }
-            if (!UNIFORM) F = mul2(F, pk(ma, mb));
-            const f2 dvx = pk(vi.x - va.x, vi.x - vb.x), dvy = pk(vi.y - va.y, vi.y - vb.y),
-                     dvz = pk(vi.z - va.z, vi.z - vb.z);
-            const f2 dot = fma2(dvz, dz, fma2(dvy, dy, mul2(dvx, dx)));
-            dr2 = fma2(F, dot, dr2);                                     // Eq. (7)
-            // L112 with c = c0 u^e, rho = rho0 u:  Pi = -alpha h c0/rho0 * (ui^e + uj^e)/(ui + uj) * min(v.r,0)/(r2+eta2);
-            // for gamma = 7 (e = 3) the quotient is ui^2 - ui uj + uj^2
-            f2 poly;
-            if (GAMMA7) {
-                poly = pk(fmaf(va.w, va.w - ui, ui2), fmaf(vb.w, vb.w - ui, ui2));
-            } else {
-                poly = pk(__fdividef(ui2 + __powf(va.w, cexp), ui + va.w), __fdividef(ui2 + __powf(vb.w, cexp), ui + vb.w));
-            }
-            float qa, qb;
-            upk(add2(r2, c_eta2), qa, qb);
-            const float rca = rcp_fast(qa), rcb = rcp_fast(qb);
-            float da, db;
-            upk(dot, da, db);
-            const f2 w = mul2(pk(fminf(da, 0.0f), fminf(db, 0.0f)), pk(rca, rcb));
-            if (MU) {
-                const float mua = ph.h * fabsf(da) * rca, mub = ph.h * fabsf(db) * rcb;
-                mumax = fmaxf(mumax, (r2a < ph.four_h2 && ma != 0.0f) ? mua : 0.0f);
-                mumax = fmaxf(mumax, (r2b < ph.four_h2 && mb != 0.0f) ? mub : 0.0f);
-            }
-            const f2 ps = pk(pi.w + ra.w, pi.w + rb.w);
-            const f2 coef = mul2(F, fma2(mul2(poly, w), c_kv, ps));      // Eq. (9) without its sign and constants
-            ax2 = fma2(coef, dx, ax2);
-            ay2 = fma2(coef, dy, ay2);
-            az2 = fma2(coef, dz, az2);
-        };
-
-        for (uint32_t bstart = 0; bstart < total; bstart += IM_BATCH) {
-            const uint32_t bend = min(total, bstart + IM_BATCH);
-            __syncthreads();                       // records of the previous batch / chunk are no longer read
-            // ---- slots of this batch: x-row r starts at a multiple of 32 (a target's window of three rows is
-            // then a whole number of 32-candidate mask words)
-            if (tid == 0) {
-                uint32_t a = 0;
-                for (int r = 0; r < 4; ++r) {
-                    const uint32_t lo = min(max(S.col_vstart[4 * r], bstart), bend);
-                    const uint32_t hi = min(max(S.col_vstart[4 * r + 4], bstart), bend);
-                    S.row_astart[r] = a;
-                    S.row_len[r] = hi - lo;
-                    a = (a + (hi - lo) + 31u) & ~31u;
-                }
-                S.row_astart[4] = a;
-            }
-            __syncthreads();
-            if (tid < IM_COLS) {
-                const int r = tid >> 2;
-                const uint32_t vs = S.col_vstart[tid], ve = S.col_vstart[tid + 1];
-                const uint32_t lo = max(vs, bstart), hi = min(ve, bend);
-                const uint32_t rlo = min(max(S.col_vstart[4 * r], bstart), bend);    // first particle of the row in the batch
-                const uint32_t gb = S.cbt[tid][0];
-                if (lo < hi) {
-                    S.stage_lo[tid] = gb + (lo - vs);
-                    S.stage_hi[tid] = gb + (hi - vs);
-                    S.stage_off[tid] = (int32_t)(S.row_astart[r] + (lo - rlo)) - (int32_t)(gb + (lo - vs));
-                } else {
-                    S.stage_lo[tid] = 0; S.stage_hi[tid] = 0; S.stage_off[tid] = 0;
-                }
-            }
-            __syncthreads();
-            // ---- stage: one bulk copy per column and array, all completing on the mbarrier
-            if (warp == 0) {
-                if (lane == 0) {
-                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-                    mbar_arrive_expect_tx(mbar, (bend - bstart) * 32u);
-                }
-                __syncwarp();
-                if (lane < IM_COLS) {
-                    const uint32_t lo = S.stage_lo[lane], cnt = S.stage_hi[lane] - lo;
-                    if (cnt) {
-                        const uint32_t a = (uint32_t)((int32_t)lo + S.stage_off[lane]);
-                        bulk_g2s(recA_addr + 16u * a, pos4 + lo, 16u * cnt, mbar);
-                        bulk_g2s(recB_addr + 16u * a, velrho4 + lo, 16u * cnt, mbar);
-                    }
-                }
-            }
-            mbar_wait(mbar, phase);
-            phase ^= 1u;
-            // ---- convert in place: tile-relative coordinates, m = |x|^2 - thr (tf32), rho -> rho/rho0; the
-            // padding slots between the rows and up to the next block of 64 become records that never hit
-            const uint32_t aend = S.row_astart[4];
-            const uint32_t nconv = (aend + 63u) & ~63u;
-            for (uint32_t a = (uint32_t)tid; a < nconv; a += IM_THREADS) {
-                int r = 0;
-#pragma unroll
-                for (int q = 1; q < 4; ++q) r += (a >= S.row_astart[q]) ? 1 : 0;
-                const uint32_t k = a - S.row_astart[r];
-                float4 ra = make_float4(0.f, 0.f, 0.f, 0.f), rb = make_float4(0.f, 0.f, 0.f, 1.f);
-                float m = __int_as_float(0x7f800000);                        // +inf: D > 0 against any target
-                if (a < aend && k < S.row_len[r]) {
-                    ra = S.recA[a];
-                    rb = S.recB[a];
-                    ra.x -= ox; ra.y -= oy; ra.z -= oz;
-                    if (!(fabsf(ra.x) <= bxy && fabsf(ra.y) <= bxy && fabsf(ra.z) <= bzz)) S.wide = 1u;
-                    m = tf32_rna(fmaf(ra.z, ra.z, fmaf(ra.y, ra.y, ra.x * ra.x)) - A.thr2);
-                    rb.w *= ph.inv_rho0;
-                    if (!UNIFORM) {
-                        const uint32_t vv = min(max(S.col_vstart[4 * r], bstart), bend) + k;   // index in the concatenation
-                        int col = 0;
-#pragma unroll
-                        for (int q = 1; q < IM_COLS; ++q) col += (vv >= S.col_vstart[q]) ? 1 : 0;
-                        const uint32_t j = S.cbt[col][0] + (vv - S.col_vstart[col]);
-                        if (__ldg(idt + j) & TYPE_BIT) rb.w = -rb.w;
-                    }
-                }
-                __syncwarp();                                // the 32 lanes of a warp cover an aligned run of 32 slots
-                const uint32_t sw = a ^ ((a >> 3) & 6u);     // swizzle: the 8 records of an mma B fragment (slots
-                S.recA[sw] = ra;                             // 2j + c + 16 q') fall on 8 different 16-byte bank groups
-                S.recB[sw] = rb;
-                S.marr[sw] = m;
-            }
-            __syncthreads();
-            const bool wide = S.wide != 0u;
-
-            if (warp_has) {
-                // ---- A rows of the distance product, handed to the lanes that hold them as mma fragments.
-                // "wide" tiles: D = m - 3e38 < 0 for every real record, +inf for the padding slots.
-                uint32_t af[4];
-                float nf[4];
-                {
-                    float4 *scratch = reinterpret_cast<float4 *>(&S.mask[warp][0][0]);
-                    float4 row = make_float4(-2.0f * xh, -2.0f * yh, -2.0f * zh, nn);
-                    if (wide) row = make_float4(0.f, 0.f, 0.f, IM_WIDE_N);
-                    if (!active) row = make_float4(0.f, 0.f, 0.f, __int_as_float(0x7f800000));
-                    scratch[lane] = row;
-                    __syncwarp();
-#pragma unroll
-                    for (int k = 0; k < 4; ++k) {
-                        const float4 r = scratch[g8 + 8 * k];
-                        const float a = qd == 0 ? r.x : (qd == 1 ? r.y : (qd == 2 ? r.z : 1.0f));
-                        af[k] = __float_as_uint(a);
-                        nf[k] = r.w;
-                    }
-                    __syncwarp();
-                }
-                // ---- one round of the mask ring per x-row of the staged region (sub-rounds if a row is longer
-                // than the ring): all lanes of a warp meet about the same number of hits in a row, so the
-                // drain that follows each filter pass keeps them busy together
-                for (int r = txmin; r <= min(txmax + 2, 3); ++r) {
-                const uint32_t e0 = S.row_astart[r] >> 5, e1 = S.row_astart[r + 1] >> 5;     // mask words of the row
-                const uint32_t e_cnt = (active && r >= tx && r <= tx + 2) ? e1 - e0 : 0u;     // ... that are this lane's
-                for (uint32_t rb0 = e0 >> 1; rb0 < ((e1 + 1u) >> 1); rb0 += IM_RB) {
-                    const uint32_t nb = min((uint32_t)IM_RB, ((e1 + 1u) >> 1) - rb0);
-                    // ---- FILTER: nb blocks of 64 slots against the warp's 32 targets
-                    for (uint32_t bi = 0; bi < nb; ++bi) {
-                        const uint32_t bb = lbase + (((rb0 + bi) * 64u) << sh);
-                        uint32_t p0 = 0, p1 = 0, p2 = 0, p3 = 0;
-#pragma unroll
-                        for (int j = 0; j < 8; ++j) {
-                            const uint32_t bf = im_lds_u32(bb + foff[j & 3] + ((uint32_t)(8 * (j >> 2)) << sh));
-                            float d0, d1, d2, d3, d4, d5, d6, d7;
-                            mma_tf32_k4(d0, d1, d2, d3, af[0], af[1], bf, nf[0], nf[0], nf[1], nf[1]);
-                            mma_tf32_k4(d4, d5, d6, d7, af[2], af[3], bf, nf[2], nf[2], nf[3], nf[3]);
-                            p0 = push_sign(d1, push_sign(d0, p0));
-                            p1 = push_sign(d3, push_sign(d2, p1));
-                            p2 = push_sign(d5, push_sign(d4, p2));
-                            p3 = push_sign(d7, push_sign(d6, p3));
-                        }
-                        const uint32_t ma = mwarp + bi * 256u + piece_addr;
-                        im_sts_u16(ma, p0);
-                        im_sts_u16(ma + 32u, p1);
-                        im_sts_u16(ma + 64u, p2);
-                        im_sts_u16(ma + 96u, p3);
-                    }
-                    __syncwarp();
-                    // ---- DRAIN.  Survey of this lane's mask words of the round: which are non-empty (nz,
-                    // bit 31 - k = word k) and how many hits they hold; the number of rounds of four pairs
-                    // is then known for the whole warp.
-                    uint32_t nz = 0, tot = 0;
-                    const uint32_t mlane = mwarp + 4u * (uint32_t)lane;          // word k of the round at mlane + 128 k
-                    for (uint32_t k = 0; k < 2u * nb; ++k) {
-                        uint32_t w = im_lds_u32(mlane + 128u * k);
-                        if ((2u * rb0 + k) - e0 >= e_cnt) w = 0u;                  // another row, or not this lane's row
-                        tot += (uint32_t)__popc(w);
-                        nz |= w ? (0x80000000u >> k) : 0u;
-                    }
-                    // a lane whose hit count is odd so far leaves its last hit alone in the LOW sub-lane; the
-                    // next hit then belongs in the HIGH one: start with the dummy partner in the low sub-lane.
-                    // cur = remaining hits of the current word (bit 31 - t = slot t of the word);
-                    // atop = shared address of recA[slot of bit 0 of cur] (bit hb is 16 hb bytes below it)
-                    uint32_t cur = odd ? 1u : 0u;
-                    uint32_t atop = dummy_addr;
-                    const uint32_t steps = __reduce_max_sync(full_mask, (tot + odd + 3u) >> 2);
-                    odd = (odd + tot) & 1u;
-                    const uint32_t atop0 = recA_addr + 16u * (rb0 * 64u + 32u * 31u + 31u);   // word k: atop0 - 512 (31 - k)
-                    const uint32_t mtop = mlane + 128u * 31u;                                   // word k at mtop - 128 (31 - k)
-                    // branch-free: the next non-empty word is read in any case (word 0 when none is left)
-                    auto pop = [&]() -> uint32_t {
-                        const uint32_t kb = bfind(nz);                                      // highest bit = lowest word
-                        const uint32_t w = im_lds_u32(mtop - 128u * (kb & 31u));
-                        const bool take = cur == 0u && nz != 0u;
-                        cur = take ? w : cur;
-                        atop = take ? atop0 - 512u * kb : atop;
-                        nz = take ? nz ^ (1u << (kb & 31u)) : nz;
-                        const uint32_t hb = bfind(cur);                                     // 0xFFFFFFFF if cur == 0
-                        const uint32_t lin = cur ? atop - 16u * hb : dummy_addr;
-                        cur &= ~(1u << (hb & 31u));
-                        return lin ^ ((lin >> 3) & 0x60u);                                  // slot swizzle, in bytes
-                    };
-                    for (uint32_t st = 0; st < steps; ++st) {
-                        const uint32_t sa = pop(), sb = pop(), sc = pop(), sd = pop();
-                        pair2(sa, sb);
-                        pair2(sc, sd);
-                    }
-                    __syncwarp();
-                }
-                }
-            }
-        }
-        if (active) {
-            float a0, a1, b0, b1, c0, c1, d0, d1;
-            upk(ax2, a0, a1); upk(ay2, b0, b1); upk(az2, c0, c1); upk(dr2, d0, d1);
-            const float k = UNIFORM ? ph.kF * ph.mass_fluid : ph.kF;
-            float ax = -k * (a0 + a1), ay = -k * (b0 + b1), az = -k * (c0 + c1);
-            const float dr = k * (d0 + d1);
-            if (fluid) { ax += ph.g[0]; ay += ph.g[1]; az += ph.g[2]; }
-            else { ax = ay = az = 0.f; }
-            acc4[i] = make_float4(ax, ay, az, dr);
-            if (MU) mu_out[i] = mumax;
-        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive((uint32_t)__cvta_generic_to_shared(&S.empty[s]));
     }
 }
 
@@ -656,16 +808,32 @@ static cudaError_t launch_mma(sph_ctx *c)
     A.cand_hi = ov.on ? ov.cand_hi : c->grid.nc[0] - 1;
     if (A.cx_end <= A.cx_first) return cudaSuccess;
     A.tx0 = A.cx_first >> 1;                       // tiles are anchored at even cell planes of the GLOBAL grid
-    const int ntx = ((A.cx_end - 1) >> 1) - A.tx0 + 1;
+    A.ntx = ((A.cx_end - 1) >> 1) - A.tx0 + 1;
     A.nty = (c->grid.nc[1] + 1) >> 1;
     A.thr2 = filter_thr(A.zb) * c->phys.h * c->phys.h;
-    const uint64_t blocks = (uint64_t)ntx * A.nty * A.nzb;
-    if (blocks == 0) return cudaSuccess;
-    kern<<<(uint32_t)blocks, IM_THREADS, sizeof(ImSmem), c->stream>>>(
+    A.tile_list = c->ia_tiles;
+    A.ctr = c->counters;
+    const uint64_t tiles = (uint64_t)A.ntx * A.nty * A.nzb;
+    if (tiles == 0) return cudaSuccess;
+    const uint32_t *cb = ov.on ? ov.cell_begin : c->cell_begin;
+    cudaError_t e = cudaMemsetAsync(c->counters + IM_CTR_NTILES, 0, 2 * sizeof(uint32_t), c->stream);
+    if (e != cudaSuccess) return e;
+    ia_tile_list_kernel<<<(uint32_t)((tiles + 255) / 256), 256, 0, c->stream>>>(cb, c->grid, A, (uint32_t)tiles, c->ia_tiles);
+    c->n_launches++;
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    const uint32_t grid = (uint32_t)(tiles < (uint64_t)NUM_SMS ? tiles : (uint64_t)NUM_SMS);
+    kern<<<grid, IM_THREADS, sizeof(ImSmem), c->stream>>>(
         ov.on ? ov.pos4 : c->pos4[c->cur], ov.on ? ov.velrho4 : c->velrho4[c->cur], ov.on ? ov.idt : c->idt[c->cur],
-        ov.on ? ov.cell_begin : c->cell_begin, ov.on ? ov.acc4 : c->acc4, c->mumax, c->grid, c->phys, A);
+        cb, ov.on ? ov.acc4 : c->acc4, c->mumax, c->grid, c->phys, A);
     c->n_launches++;
     return cudaGetLastError();
+}
+
+// capacity of the tile list for a grid and z-block
+size_t interact_mma_tile_capacity(const int nc[3], int zb)
+{
+    return (size_t)((nc[0] + 1) / 2 + 1) * (size_t)((nc[1] + 1) / 2) * (size_t)((nc[2] + zb - 1) / zb);
 }
 
 template <bool MU>

@@ -17,7 +17,7 @@ size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 struct Layout {
     size_t pos4[2], velrho4[2], velrhoM1[2], idt[2], acc4, mumax, dt_red, kv[2], keyword, hist, tile_state, counters,
         cell_begin, cell_loc, gap_list, mig_tile, mig_grp, mig_off, scratch64, slab_begin, halo_range, halo_offset, halo_pos4, halo_velrho4, halo_idt,
-        migrants, mig_total, mig_count, prev_init, flags, total;
+        migrants, mig_total, mig_count, prev_init, flags, ia_tiles, total;
 };
 
 bool grid_of(const sph_params *p, int nc[3], uint64_t *ncells)
@@ -36,6 +36,17 @@ bool grid_of(const sph_params *p, int nc[3], uint64_t *ncells)
     }
     *ncells = tot;
     return true;
+}
+
+// cells per z-block of a tile of the production interaction kernel: 2 x 2 columns x zm cells fill an
+// item's target list
+int mma_zblock(const sph_params *p)
+{
+    double ppc = pow(2.0 * (double)p->h / (double)p->dp, 3.0);
+    int zm = (int)floor((double)interact_mma_targets() * 0.97 / (4.0 * (ppc > 0.05 ? ppc : 0.05)));
+    if (zm < 1) zm = 1;
+    if (zm > interact_mma_zmax()) zm = interact_mma_zmax();
+    return zm;
 }
 
 bool make_layout(const sph_params *p, uint64_t n, int max_slabs, Layout *L)
@@ -82,6 +93,7 @@ bool make_layout(const sph_params *p, uint64_t n, int max_slabs, Layout *L)
     L->mig_count = take(4 * 2 * SPH_MAX_SLABS);
     L->prev_init = take(nn);
     L->flags = take(4);
+    L->ia_tiles = take(4 * interact_mma_tile_capacity(nc, mma_zblock(p)));
     L->total = off;
     return true;
 }
@@ -313,11 +325,8 @@ int sph_init(sph_ctx **out, const sph_params *p, const sph_particles *part, int 
     if (zb < 1) zb = 1;
     if (zb > 32) zb = 32;
     c->zblock = zb;
-    // production kernel: a tile of 2 x 2 columns x zm cells fills the CTA's threads with targets
-    int zm = (int)floor((double)interact_mma_threads() * 0.97 / (4.0 * (ppc > 0.05 ? ppc : 0.05)));
-    if (zm < 1) zm = 1;
-    if (zm > interact_mma_zmax()) zm = interact_mma_zmax();
-    c->zblock_mma = zm;
+    c->zblock_mma = mma_zblock(p);
+    c->ia_tiles = (uint32_t *)(w + L.ia_tiles);
 
     c->last_cuda_error[0] = 0;
     c->id_order = true;

@@ -134,6 +134,7 @@ struct sph_ctx {
     sph::StageTimer timer;
     sph::IaOverride ia_ov;     // off except inside sph_interact_slab
     uint32_t *cell_loc;        // ncells+1: cell table a slab rebuilds from its own + halo particles
+    uint32_t *ia_tiles;        // list of the non-empty tiles of the production interaction kernel
 };
 
 namespace sph {
@@ -166,7 +167,8 @@ cudaError_t launch_fma_peak(sph_ctx *c, int variant, int iters, int blocks, floa
 cudaError_t configure_interact();
 cudaError_t configure_interact_mma();
 cudaError_t launch_interact_mma(sph_ctx *c, bool with_mu);
-int interact_mma_threads();
+int interact_mma_targets();
+size_t interact_mma_tile_capacity(const int nc[3], int zb);
 int interact_mma_zmax();
 cudaError_t configure_sort();
 
