@@ -51,16 +51,25 @@ namespace sph {
 #ifndef SPH_IM_PRODUCERS
 #define SPH_IM_PRODUCERS 4
 #endif
+#ifndef SPH_IM_SLEEP_NS
+#define SPH_IM_SLEEP_NS 256
+#endif
 #ifndef SPH_IM_RB
 #define SPH_IM_RB 9
 #endif
 constexpr int IM_NC = SPH_IM_CONSUMERS;      // consumer warps
 constexpr int IM_NP = SPH_IM_PRODUCERS;       // producer warps
 constexpr int IM_THREADS = 32 * (IM_NC + IM_NP);
-constexpr int IM_MAXT = 352;                 // targets per item: 2 x 2 x 3 cells x 27 particles = 324
+#ifndef SPH_IM_MAXT
+#define SPH_IM_MAXT 352
+#endif
+#ifndef SPH_IM_CAP
+#define SPH_IM_CAP 2304
+#endif
+constexpr int IM_MAXT = SPH_IM_MAXT;                 // targets per item: 2 x 2 x 3 cells x 27 particles = 324
 constexpr int IM_COLS = 16;                  // staged columns: 4 x 4
 constexpr int IM_ZMAX = 6;                   // max cells per z-block (tf32 model: |z| <= (zb + 2) h)
-constexpr int IM_CAP = 2304;                 // staged record slots per batch = 36 blocks of 64
+constexpr int IM_CAP = SPH_IM_CAP;                 // staged record slots per batch = 36 blocks of 64
 constexpr int IM_BATCH = IM_CAP - 128;       // particles per batch (16 x 5 x 27 = 2160): the 4 x-rows start at multiples
                                              // of 32 slots, which costs up to 4 x 31 padding slots
 constexpr int IM_RB = SPH_IM_RB;             // mask ring: blocks of 64 candidates per warp per round
@@ -97,6 +106,7 @@ struct __align__(1024) ImSmem {
     uint32_t bcnt[32];                       // target ordering: bucket counts, then bucket starts
     uint32_t tkey[IM_MAXT];                  // target ordering: bucket | rank << 8 | own column << 28
     uint32_t tidx[IM_MAXT];                  // target ordering: global index
+    uint32_t tnext[IM_MAXT];                 // target list of the item being prepared
     uint32_t row_len[4];
     uint32_t tile;                           // the tile the producers work on
     unsigned long long full[IM_STAGES], empty[IM_STAGES], tma;
@@ -172,14 +182,17 @@ __device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t mbar, uint32_t by
 {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar), "r"(bytes) : "memory");
 }
-__device__ __forceinline__ void mbar_wait(uint32_t mbar, uint32_t parity)
+__device__ __forceinline__ bool mbar_try(uint32_t mbar, uint32_t parity)
 {
     uint32_t done;
-    do {
-        // the thread sleeps until the phase completes or the time hint (ns) runs out: no issue slots are spent polling
-        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-                     : "=r"(done) : "r"(mbar), "r"(parity), "r"(20000u) : "memory");
-    } while (!done);
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(done) : "r"(mbar), "r"(parity) : "memory");
+    return done != 0u;
+}
+// waiting warps sleep between polls so that they do not take issue slots from the working ones
+__device__ __forceinline__ void mbar_wait(uint32_t mbar, uint32_t parity)
+{
+    while (!mbar_try(mbar, parity)) __nanosleep(SPH_IM_SLEEP_NS);
 }
 // 1-D bulk asynchronous copy global -> shared (SASS: UBLKCP); bytes % 16 == 0, both sides 16-byte aligned
 __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t mbar)
@@ -344,52 +357,12 @@ __device__ __forceinline__ void im_produce(ImSmem &S, const float4 *__restrict__
                 const uint32_t bend = min(total, bstart + IM_BATCH);
                 const uint32_t s = it & 1u, use = it >> 1;
                 ImStage &T = S.st[s];
-                mbar_wait((uint32_t)__cvta_generic_to_shared(&S.empty[s]), (use & 1u) ^ 1u);
-                // a later batch adds to what the previous item wrote: wait until that item has drained
-                if (bstart > 0) mbar_wait((uint32_t)__cvta_generic_to_shared(&S.empty[s ^ 1u]), ((it - 1u) >> 1) & 1u);
-                const uint32_t recA_addr = (uint32_t)__cvta_generic_to_shared(T.recA);
-                const uint32_t recB_addr = (uint32_t)__cvta_generic_to_shared(T.recB);
-
-                // ---- slots of this batch: x-row r starts at a multiple of 32 (a target's window of three rows
-                // is then a whole number of 32-candidate mask words)
-                if (ptid == 0) {
-                    uint32_t a = 0;
-                    for (int r = 0; r < 4; ++r) {
-                        const uint32_t lo = min(max(S.col_vstart[4 * r], bstart), bend);
-                        const uint32_t hi = min(max(S.col_vstart[4 * r + 4], bstart), bend);
-                        T.row_astart[r] = a;
-                        S.row_len[r] = hi - lo;
-                        a = (a + (hi - lo) + 31u) & ~31u;
-                    }
-                    T.row_astart[4] = a;
-                    T.ntargets = nT;
-                    T.chunk_ctr = 0u;
-                    T.wide = 0u;
-                    T.accumulate = bstart > 0 ? 1u : 0u;
-                    T.exit = 0u;
-                    T.ox = ox; T.oy = oy; T.oz = oz; T.bxy = bxy; T.bzz = bzz;
-                    mbar_arrive_expect_tx(tma, (bend - bstart) * 32u);
-                }
-                if (ptid < 32) S.bcnt[ptid] = 0u;
-                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");    // generic writes of the last use < bulk copies
-                im_pbar();
-                // ---- stage: one bulk copy per column and array, all completing on the mbarrier
-                if (ptid < IM_COLS) {
-                    const int r = ptid >> 2;
-                    const uint32_t vs = S.col_vstart[ptid], ve = S.col_vstart[ptid + 1];
-                    const uint32_t lo = max(vs, bstart), hi = min(ve, bend);
-                    const uint32_t rlo = min(max(S.col_vstart[4 * r], bstart), bend);    // first particle of the row in the batch
-                    if (lo < hi) {
-                        const uint32_t gl = S.cbt[ptid][0] + (lo - vs);
-                        const uint32_t a = T.row_astart[r] + (lo - rlo);
-                        bulk_g2s(recA_addr + 16u * a, pos4 + gl, 16u * (hi - lo), tma);
-                        bulk_g2s(recB_addr + 16u * a, velrho4 + gl, 16u * (hi - lo), tma);
-                    }
-                }
-                // ---- meanwhile: order the targets by (x-row, position inside the cell along x).  How many hits
+                // ---- before the stage is free: order the targets by (x-row, position inside the cell along x).  How many hits
                 // a target meets in each x-row of the staged region depends on where it sits in its cell along
                 // x; the drain works row by row, so a warp whose lanes share that position keeps all its lanes
                 // busy in every row.  The order of a target's own sum does not depend on its lane.
+                if (ptid < 32) S.bcnt[ptid] = 0u;
+                im_pbar();
                 for (uint32_t q = ptid; q < nT; q += PT) {
                     const uint32_t tq = t0 + q;
                     int tc = 0;
@@ -417,8 +390,51 @@ __device__ __forceinline__ void im_produce(ImSmem &S, const float4 *__restrict__
                 im_pbar();
                 for (uint32_t q = ptid; q < nT; q += PT) {
                     const uint32_t k = S.tkey[q];
-                    T.tglob[S.bcnt[k & 31u] + ((k >> 8) & 0xFFFFFu)] = S.tidx[q] | (k & 0x30000000u);
+                    S.tnext[S.bcnt[k & 31u] + ((k >> 8) & 0xFFFFFu)] = S.tidx[q] | (k & 0x30000000u);
                 }
+                mbar_wait((uint32_t)__cvta_generic_to_shared(&S.empty[s]), (use & 1u) ^ 1u);
+                // a later batch adds to what the previous item wrote: wait until that item has drained
+                if (bstart > 0) mbar_wait((uint32_t)__cvta_generic_to_shared(&S.empty[s ^ 1u]), ((it - 1u) >> 1) & 1u);
+                const uint32_t recA_addr = (uint32_t)__cvta_generic_to_shared(T.recA);
+                const uint32_t recB_addr = (uint32_t)__cvta_generic_to_shared(T.recB);
+
+                // ---- slots of this batch: x-row r starts at a multiple of 32 (a target's window of three rows
+                // is then a whole number of 32-candidate mask words)
+                if (ptid == 0) {
+                    uint32_t a = 0;
+                    for (int r = 0; r < 4; ++r) {
+                        const uint32_t lo = min(max(S.col_vstart[4 * r], bstart), bend);
+                        const uint32_t hi = min(max(S.col_vstart[4 * r + 4], bstart), bend);
+                        T.row_astart[r] = a;
+                        S.row_len[r] = hi - lo;
+                        a = (a + (hi - lo) + 31u) & ~31u;
+                    }
+                    T.row_astart[4] = a;
+                    T.ntargets = nT;
+                    T.chunk_ctr = 0u;
+                    T.wide = 0u;
+                    T.accumulate = bstart > 0 ? 1u : 0u;
+                    T.exit = 0u;
+                    T.ox = ox; T.oy = oy; T.oz = oz; T.bxy = bxy; T.bzz = bzz;
+                    mbar_arrive_expect_tx(tma, (bend - bstart) * 32u);
+                }
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");    // generic writes of the last use < bulk copies
+                im_pbar();
+                // ---- stage: one bulk copy per column and array, all completing on the mbarrier
+                if (ptid < IM_COLS) {
+                    const int r = ptid >> 2;
+                    const uint32_t vs = S.col_vstart[ptid], ve = S.col_vstart[ptid + 1];
+                    const uint32_t lo = max(vs, bstart), hi = min(ve, bend);
+                    const uint32_t rlo = min(max(S.col_vstart[4 * r], bstart), bend);    // first particle of the row in the batch
+                    if (lo < hi) {
+                        const uint32_t gl = S.cbt[ptid][0] + (lo - vs);
+                        const uint32_t a = T.row_astart[r] + (lo - rlo);
+                        bulk_g2s(recA_addr + 16u * a, pos4 + gl, 16u * (hi - lo), tma);
+                        bulk_g2s(recB_addr + 16u * a, velrho4 + gl, 16u * (hi - lo), tma);
+                    }
+                }
+                // ---- the target list, prepared before the stage was acquired
+                for (uint32_t q = ptid; q < nT; q += PT) T.tglob[q] = S.tnext[q];
                 mbar_wait(tma, tma_phase);
                 tma_phase ^= 1u;
                 // ---- convert in place: tile-relative coordinates, m = |x|^2 - thr (tf32), rho -> rho/rho0; the
