@@ -98,7 +98,8 @@ struct __align__(1024) ImStage {    // recA at a multiple of 1024 B: the slot sw
 
 struct __align__(1024) ImSmem {
     ImStage st[IM_STAGES];
-    uint32_t mask[IM_NC][IM_RB][64];         // per consumer warp and ring slot: [half][target lane] hit masks of 32 candidates
+    uint32_t mask[IM_NC][IM_RB * 64 + 32];   // per consumer warp and ring slot: [half][target lane] hit masks of 32 candidates;
+                                             // + one row of empty words (the sentinel that ends every lane's word list)
     // producer-private
     uint32_t cbt[IM_COLS][IM_ZMAX + 3];      // cell_begin of the 16 columns over [zlo, zhi]
     uint32_t col_vstart[IM_COLS + 1];        // virtual start of each column in the concatenation
@@ -696,24 +697,27 @@ __device__ __forceinline__ void im_chunk(ImStage &T, uint32_t mwarp, uint32_t ch
                 odd = (odd + tot) & 1u;
                 const uint32_t atop0 = recA_addr + 16u * (rb0 * 64u + 32u * 31u + 31u);   // word k: atop0 - 512 (31 - k)
                 const uint32_t mtop = mlane + 128u * 31u;                                   // word k at mtop - 128 (31 - k)
+                // the word after the ring's last one is always empty: its bit stays in nz, so that a lane that has
+                // used up its words keeps fetching an empty word (no test for "none left" in the pop)
+                constexpr uint32_t sent = 0x80000000u >> (2 * IM_RB);
+                nz |= sent;
                 uint32_t nxtw, nxta;
                 {
                     const uint32_t kb = bfind(nz);                                      // highest bit = lowest word
-                    const uint32_t w = im_lds_u32(mtop - 128u * (kb & 31u));
-                    nxtw = nz ? w : 0u;
+                    nxtw = im_lds_u32(mtop - 128u * kb);
                     nxta = atop0 - 512u * kb;
-                    nz &= ~(1u << (kb & 31u));
+                    nz = (nz & ~(1u << kb)) | sent;
                 }
-                // branch-free: the word after next is read in any case (word 0 when none is left)
+                // branch-free: the word after next is read in any case
                 auto pop = [&]() -> uint32_t {
                     const uint32_t kb = bfind(nz);
-                    const uint32_t w = im_lds_u32(mtop - 128u * (kb & 31u));
+                    const uint32_t w = im_lds_u32(mtop - 128u * kb);
                     const bool take = cur == 0u;
                     cur = take ? nxtw : cur;
                     atop = take ? nxta : atop;
-                    nxtw = take ? (nz ? w : 0u) : nxtw;
+                    nxtw = take ? w : nxtw;
                     nxta = take ? atop0 - 512u * kb : nxta;
-                    nz = take ? nz & ~(1u << (kb & 31u)) : nz;
+                    nz = take ? (nz & ~(1u << kb)) | sent : nz;
                     const uint32_t hb = bfind(cur);                                     // 0xFFFFFFFF if cur == 0
                     const uint32_t lin = cur ? atop - 16u * hb : dummy_addr;
                     cur &= ~(1u << (hb & 31u));
@@ -760,6 +764,7 @@ interact_mma_kernel(const float4 *__restrict__ pos4, const float4 *__restrict__ 
     ImSmem &S = *reinterpret_cast<ImSmem *>(im_raw);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
+    for (int k = tid; k < IM_NC * 32; k += IM_THREADS) S.mask[k >> 5][IM_RB * 64 + (k & 31)] = 0u;
     if (tid == 0) {
         for (int s = 0; s < IM_STAGES; ++s) {
             mbar_init((uint32_t)__cvta_generic_to_shared(&S.full[s]), 1u);
@@ -773,10 +778,16 @@ interact_mma_kernel(const float4 *__restrict__ pos4, const float4 *__restrict__ 
     __syncthreads();
 
     if (warp < IM_NP) {
+#ifdef SPH_IM_REGS_CONSUMER
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(SPH_IM_REGS_PRODUCER));   // registers go to the consumers
+#endif
         im_produce<UNIFORM>(S, pos4, velrho4, idt, cell_begin, g, ph, A);
         return;
     }
-    const uint32_t mwarp = (uint32_t)__cvta_generic_to_shared(&S.mask[warp - IM_NP][0][0]);
+#ifdef SPH_IM_REGS_CONSUMER
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(SPH_IM_REGS_CONSUMER));
+#endif
+    const uint32_t mwarp = (uint32_t)__cvta_generic_to_shared(&S.mask[warp - IM_NP][0]);
     for (uint32_t it = 0;; ++it) {
         const uint32_t s = it & 1u;
         ImStage &T = S.st[s];
