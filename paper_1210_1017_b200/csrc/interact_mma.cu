@@ -93,6 +93,8 @@ struct __align__(1024) ImStage {    // recA at a multiple of 1024 B: the slot sw
     uint32_t wide;                           // some record lies outside the tf32 error model
     uint32_t accumulate;                     // add to the rates already in memory (second and later batches)
     uint32_t exit;                           // no more work
+    uint32_t first_chunk;                    // the chunk handed out first: the one whose targets lie in both x-rows of
+                                             // the tile needs four candidate rows instead of three and takes longest
     float ox, oy, oz, bxy, bzz;              // tile origin and the bounds of the tf32 error model
 };
 
@@ -200,6 +202,11 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t
 {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  ::"r"(dst), "l"(src), "r"(bytes), "r"(mbar) : "memory");
+}
+// the same range into L2 only
+__device__ __forceinline__ void bulk_prefetch_l2(const void *src, uint32_t bytes)
+{
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
 }
 __device__ __forceinline__ float tf32_rna(float x)
 {
@@ -393,6 +400,17 @@ __device__ __forceinline__ void im_produce(ImSmem &S, const float4 *__restrict__
                     const uint32_t k = S.tkey[q];
                     S.tnext[S.bcnt[k & 31u] + ((k >> 8) & 0xFFFFFu)] = S.tidx[q] | (k & 0x30000000u);
                 }
+                // ... and pull the item's records into L2, so that the bulk copies issued once the stage is free
+                // do not wait for HBM
+                if (ptid < IM_COLS) {
+                    const uint32_t vs = S.col_vstart[ptid], ve = S.col_vstart[ptid + 1];
+                    const uint32_t lo = max(vs, bstart), hi = min(ve, bend);
+                    if (lo < hi) {
+                        const uint32_t gl = S.cbt[ptid][0] + (lo - vs);
+                        bulk_prefetch_l2(pos4 + gl, 16u * (hi - lo));
+                        bulk_prefetch_l2(velrho4 + gl, 16u * (hi - lo));
+                    }
+                }
                 mbar_wait((uint32_t)__cvta_generic_to_shared(&S.empty[s]), (use & 1u) ^ 1u);
                 // a later batch adds to what the previous item wrote: wait until that item has drained
                 if (bstart > 0) mbar_wait((uint32_t)__cvta_generic_to_shared(&S.empty[s ^ 1u]), ((it - 1u) >> 1) & 1u);
@@ -416,6 +434,10 @@ __device__ __forceinline__ void im_produce(ImSmem &S, const float4 *__restrict__
                     T.wide = 0u;
                     T.accumulate = bstart > 0 ? 1u : 0u;
                     T.exit = 0u;
+                    {
+                        const uint32_t n0 = min(max(S.tstart[2], t0), t0 + nT) - t0;      // targets of the first x-row
+                        T.first_chunk = (n0 & 31u) && n0 < nT ? n0 >> 5 : 0u;
+                    }
                     T.ox = ox; T.oy = oy; T.oz = oz; T.bxy = bxy; T.bzz = bzz;
                     mbar_arrive_expect_tx(tma, (bend - bstart) * 32u);
                 }
@@ -799,6 +821,8 @@ interact_mma_kernel(const float4 *__restrict__ pos4, const float4 *__restrict__ 
             if (lane == 0) c = atomicAdd(&T.chunk_ctr, 1u);
             c = __shfl_sync(0xffffffffu, c, 0);
             if (c >= nchunks) break;
+            const uint32_t fc = T.first_chunk;
+            c = c == 0u ? fc : (c <= fc ? c - 1u : c);
             im_chunk<KERNEL, UNIFORM, GAMMA7, MU>(T, mwarp, c, pos4, velrho4, idt, acc4, mu_out, ph);
         }
         __syncwarp();
