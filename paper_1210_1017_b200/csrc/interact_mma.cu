@@ -261,11 +261,22 @@ __device__ __forceinline__ void im_tile_coords(uint32_t b, const ImArgs &A, int 
 }
 
 // ---- list of the non-empty tiles (most of a dam-break tank holds no particle) ------------------------
+// Listed z-block fastest, then y inside strips of IM_STRIP tiles, then x, then strip: tiles that share
+// staged columns are handed out close in time, so the second reader of a column finds it in L2.
+constexpr int IM_STRIP = 8;
 __global__ void __launch_bounds__(256)
-ia_tile_list_kernel(const uint32_t *__restrict__ cell_begin, GridC g, ImArgs A, uint32_t ntiles, uint32_t *list)
+ia_tile_list_kernel(const uint32_t *__restrict__ cell_begin, GridC g, ImArgs A, uint32_t nthreads, uint32_t *list)
 {
-    const uint32_t b = blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= ntiles) return;
+    uint32_t q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= nthreads) return;
+    const uint32_t bz = q % (uint32_t)A.nzb;
+    q /= (uint32_t)A.nzb;
+    const uint32_t tyl = q % IM_STRIP;
+    q /= IM_STRIP;
+    const uint32_t tx = q % (uint32_t)A.ntx, strip = q / (uint32_t)A.ntx;
+    const uint32_t ty = strip * IM_STRIP + tyl;
+    if (ty >= (uint32_t)A.nty) return;
+    const uint32_t b = (tx * (uint32_t)A.nty + ty) * (uint32_t)A.nzb + bz;
     int cx0, cy0, cz0;
     im_tile_coords(b, A, cx0, cy0, cz0);
     const int cz1 = min(cz0 + A.zb, g.nc[2]);
@@ -278,7 +289,7 @@ ia_tile_list_kernel(const uint32_t *__restrict__ cell_begin, GridC g, ImArgs A, 
             any |= cell_begin[colbase + cz1] - cell_begin[colbase + cz0];
         }
     }
-    if (any) list[atomicAdd(A.ctr + IM_CTR_NTILES, 1u)] = b;     // any order: a tile's result does not depend on it
+    if (any) list[atomicAdd(A.ctr + IM_CTR_NTILES, 1u)] = b;     // approximate order: a tile's result does not depend on it
 }
 
 // ---- producers: IM_NP warps working as one group (named barrier 1) -----------------------------------
@@ -869,7 +880,8 @@ static cudaError_t launch_mma(sph_ctx *c)
     const uint32_t *cb = ov.on ? ov.cell_begin : c->cell_begin;
     cudaError_t e = cudaMemsetAsync(c->counters + IM_CTR_NTILES, 0, 2 * sizeof(uint32_t), c->stream);
     if (e != cudaSuccess) return e;
-    ia_tile_list_kernel<<<(uint32_t)((tiles + 255) / 256), 256, 0, c->stream>>>(cb, c->grid, A, (uint32_t)tiles, c->ia_tiles);
+    const uint64_t lthreads = (uint64_t)((A.nty + IM_STRIP - 1) / IM_STRIP) * A.ntx * IM_STRIP * A.nzb;
+    ia_tile_list_kernel<<<(uint32_t)((lthreads + 255) / 256), 256, 0, c->stream>>>(cb, c->grid, A, (uint32_t)lthreads, c->ia_tiles);
     c->n_launches++;
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
