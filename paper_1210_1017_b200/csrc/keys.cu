@@ -96,7 +96,6 @@ keys_kernel(uint32_t n, const float4 *__restrict__ pos4, const uint32_t *__restr
     }
 
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const uint32_t lt_mask = (1u << lane) - 1u;
     constexpr uint32_t WCHUNK = 32 * KEYS_IPT;
     const uint32_t stride = gridDim.x * (blockDim.x >> 5) * WCHUNK;
     // a warp owns WCHUNK consecutive particles per iteration; the loop bound is warp-uniform, so
@@ -119,7 +118,9 @@ keys_kernel(uint32_t n, const float4 *__restrict__ pos4, const uint32_t *__restr
             uint32_t cell = 0;
             if (valid) {
                 const uint32_t id = w[k] & ID_MASK;
-                if (!(isfinite(p[k].x) && isfinite(p[k].y) && isfinite(p[k].z))) atomicOr(flags, FLAG_NONFINITE);
+                // one test for the three coordinates: NaN and Inf survive the sum (so does an overflow of finite
+                // values beyond 1e38 m, which is no position either)
+                if (!(fabsf(p[k].x) + fabsf(p[k].y) + fabsf(p[k].z) < __int_as_float(0x7f800000))) atomicOr(flags, FLAG_NONFINITE);
                 const int cx = cell_coord(p[k].x, g.min[0], g.inv_cell, g.nc[0]);
                 const int cy = cell_coord(p[k].y, g.min[1], g.inv_cell, g.nc[1]);
                 const int cz = cell_coord(p[k].z, g.min[2], g.inv_cell, g.nc[2]);
@@ -150,32 +151,19 @@ keys_kernel(uint32_t n, const float4 *__restrict__ pos4, const uint32_t *__restr
                 const uint32_t tag = lab | (mig << 2);
                 kv_by_id[id] = make_uint2((tag << TAG_SHIFT) | cell, ((uint32_t)prev << 28) | i);
             }
-            // digit histograms in shared memory.  One digit in the whole warp (the usual case for the
-            // upper digits of a running simulation): one atomic.  A few runs of equal digits: hardware
-            // MATCH.ANY (its cost grows with the number of distinct values) and one atomic per run.
-            // Otherwise (random keys): one plain shared-memory atomic per key - with ~28 distinct
-            // digits among 32 lanes they hardly collide, measured 2.4 cycles per warp instruction.
-            const uint32_t vmask = __ballot_sync(0xffffffffu, valid);
-            // valid lanes are a prefix of the warp, so lane 0 speaks for a warp that has any
-            const uint32_t c0 = __shfl_sync(0xffffffffu, cell, 0);
-            const bool upper_uniform = __all_sync(0xffffffffu, !valid || (cell >> 8) == (c0 >> 8));
+            // digit histograms in shared memory, all passes at once from the runs of equal CELLS in the warp:
+            // the lane that starts a run adds the run's length to the run's digit of every pass.  In a
+            // running simulation the 32 particles of a row lie in one to three cells (a handful of atomics
+            // per row); random keys make every lane a run of one (one atomic per key and pass, which hardly
+            // collide with ~28 distinct digits among 32 lanes).
+            const uint32_t key = valid ? cell : 0xFFFFFFFFu;           // invalid lanes are a suffix: one last run
+            const uint32_t left = __shfl_up_sync(0xffffffffu, key, 1);
+            const uint32_t heads = __ballot_sync(0xffffffffu, lane == 0 || key != left);
+            if (valid && ((heads >> lane) & 1u)) {
+                const uint32_t after = heads & ~((2u << lane) - 1u);   // run heads to the right of this lane
+                const uint32_t len = (after ? (uint32_t)__ffs(after) - 1u : 32u) - lane;
 #pragma unroll
-            for (int q = 0; q < PASSES; ++q) {
-                if (q > 0 && upper_uniform) {             // one test covers all the upper digits
-                    if (lane == 0 && vmask) atomicAdd(&s_hist[q * 256 + ((c0 >> (8 * q)) & 255u)], __popc(vmask));
-                    continue;
-                }
-                const uint32_t d = valid ? ((cell >> (8 * q)) & 255u) : 256u;
-                const uint32_t prev = __shfl_up_sync(0xffffffffu, d, 1);
-                const uint32_t runs = __ballot_sync(0xffffffffu, d != prev);   // lane 0: compares with itself
-                if (runs == 0) {
-                    if (lane == 0 && vmask) atomicAdd(&s_hist[q * 256 + d], __popc(vmask));
-                } else if (__popc(runs) <= MATCH_MAX_RUNS) {
-                    const uint32_t m = __match_any_sync(0xffffffffu, d);
-                    if (valid && (m & lt_mask) == 0) atomicAdd(&s_hist[q * 256 + d], __popc(m));
-                } else if (valid) {
-                    atomicAdd(&s_hist[q * 256 + d], 1u);
-                }
+                for (int q = 0; q < PASSES; ++q) atomicAdd(&s_hist[q * 256 + ((cell >> (8 * q)) & 255u)], len);
             }
         }
     }
@@ -194,7 +182,17 @@ cudaError_t launch_keys(sph_ctx *c)
     if (n == 0) return cudaSuccess;
     int prev_mode = c->have_prev_init ? 2 : (c->have_prev_ranges ? 1 : 0);
     uint32_t blocks = (n + 256 * KEYS_IPT - 1) / (256 * KEYS_IPT);
-    uint32_t cap = NUM_SMS * 8;
+    // grid-stride loop: exactly one resident wave, so that no SM waits for a second, partial one
+    int per_sm = 0;
+    auto occ = [&](auto kern) { return cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, 256, 0); };
+    switch (c->passes) {
+    case 1: e = occ(keys_kernel<1>); break;
+    case 2: e = occ(keys_kernel<2>); break;
+    case 3: e = occ(keys_kernel<3>); break;
+    default: e = occ(keys_kernel<4>); break;
+    }
+    if (e != cudaSuccess) return e;
+    uint32_t cap = NUM_SMS * (uint32_t)(per_sm > 0 ? per_sm : 1);
     if (blocks > cap) blocks = cap;
     const float4 *pos4 = c->pos4[c->cur];
     const uint32_t *idt = c->idt[c->cur];
