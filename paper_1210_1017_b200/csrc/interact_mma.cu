@@ -106,8 +106,8 @@ struct __align__(1024) ImSmem {
     uint32_t cbt[IM_COLS][IM_ZMAX + 3];      // cell_begin of the 16 columns over [zlo, zhi]
     uint32_t col_vstart[IM_COLS + 1];        // virtual start of each column in the concatenation
     uint32_t tstart[5], tbase[4], tcnt[4];   // target ranges of the 2 x 2 own columns
-    uint32_t bcnt[32];                       // target ordering: bucket counts, then bucket starts
-    uint32_t tkey[IM_MAXT];                  // target ordering: bucket | rank << 8 | own column << 28
+    uint32_t wcnt[IM_NP][32];                // target ordering: per producer warp and bucket, counts, then next slots
+    uint32_t tkey[IM_MAXT];                  // target ordering: bucket | own column << 28
     uint32_t tidx[IM_MAXT];                  // target ordering: global index
     uint32_t tnext[IM_MAXT];                 // target list of the item being prepared
     uint32_t row_len[4];
@@ -376,40 +376,60 @@ __device__ __forceinline__ void im_produce(ImSmem &S, const float4 *__restrict__
                 const uint32_t bend = min(total, bstart + IM_BATCH);
                 const uint32_t s = it & 1u, use = it >> 1;
                 ImStage &T = S.st[s];
-                // ---- before the stage is free: order the targets by (x-row, position inside the cell along x).  How many hits
-                // a target meets in each x-row of the staged region depends on where it sits in its cell along
-                // x; the drain works row by row, so a warp whose lanes share that position keeps all its lanes
-                // busy in every row.  The order of a target's own sum does not depend on its lane.
-                if (ptid < 32) S.bcnt[ptid] = 0u;
-                im_pbar();
-                for (uint32_t q = ptid; q < nT; q += PT) {
-                    const uint32_t tq = t0 + q;
-                    int tc = 0;
+                // ---- before the stage is free: order the targets by (x-row, position inside the cell along x), and
+                // inside such a bucket by their sorted index (a STABLE counting sort: every producer warp ranks a
+                // contiguous piece of the targets, so that bucket order = index order and the list is the same in
+                // every run).  How many hits a target meets in each x-row of the staged region depends on where
+                // it sits in its cell along x; the drain works row by row, so a warp whose lanes share that
+                // position keeps all its lanes busy in every row.  The order of a target's own sum does not
+                // depend on its lane.
+                const uint32_t per = ((nT + IM_NP - 1) / IM_NP + 31u) & ~31u;          // targets per producer warp
+                const uint32_t q_lo = (uint32_t)pwarp * per, q_hi = min(nT, q_lo + per);
+                S.wcnt[pwarp][lane] = 0u;
+                __syncwarp();
+                for (uint32_t q = q_lo + lane; q < q_lo + per; q += 32) {
+                    uint32_t bk = 64u + lane;                                           // no target: a key of its own
+                    if (q < q_hi) {
+                        const uint32_t tq = t0 + q;
+                        int tc = 0;
 #pragma unroll
-                    for (int t = 1; t < 4; ++t) tc += (tq >= S.tstart[t]) ? 1 : 0;
-                    const uint32_t i = S.tbase[tc] + (tq - S.tstart[tc]);
-                    const float px = __ldg(reinterpret_cast<const float *>(pos4 + i)) - ox;    // column tc >> 1 spans
-                    const float ph16 = (px - (float)((tc >> 1) - 1) * cell) * (16.0f / cell);     // [(tx-1) cell, tx cell)
-                    const uint32_t bk = (uint32_t)(tc >> 1) * 16u + (uint32_t)min(max(__float2int_rd(ph16), 0), 15);
-                    const uint32_t rk = atomicAdd(&S.bcnt[bk], 1u);
-                    S.tkey[q] = bk | (rk << 8) | ((uint32_t)tc << 28);
-                    S.tidx[q] = i;
+                        for (int t = 1; t < 4; ++t) tc += (tq >= S.tstart[t]) ? 1 : 0;
+                        const uint32_t i = S.tbase[tc] + (tq - S.tstart[tc]);
+                        const float px = __ldg(reinterpret_cast<const float *>(pos4 + i)) - ox;    // column tc >> 1 spans
+                        const float ph16 = (px - (float)((tc >> 1) - 1) * cell) * (16.0f / cell);     // [(tx-1) cell, tx cell)
+                        bk = (uint32_t)(tc >> 1) * 16u + (uint32_t)min(max(__float2int_rd(ph16), 0), 15);
+                        S.tkey[q] = bk | ((uint32_t)tc << 28);
+                        S.tidx[q] = i;
+                    }
+                    const uint32_t m = __match_any_sync(full_mask, bk);
+                    if (q < q_hi && (m & ((1u << lane) - 1u)) == 0u) S.wcnt[pwarp][bk] += (uint32_t)__popc(m);
+                    __syncwarp();
                 }
                 im_pbar();
-                if (pwarp == 0) {
-                    const uint32_t v = S.bcnt[lane];
-                    uint32_t inc = v;
+                if (pwarp == 0) {                     // lane = bucket: first slot of every (bucket, producer warp)
+                    uint32_t run = 0;
+                    uint32_t part[IM_NP];
+#pragma unroll
+                    for (int w = 0; w < IM_NP; ++w) { part[w] = run; run += S.wcnt[w][lane]; }
+                    uint32_t inc = run;
 #pragma unroll
                     for (int o = 1; o < 32; o <<= 1) {
                         const uint32_t t = __shfl_up_sync(full_mask, inc, o);
                         if (lane >= o) inc += t;
                     }
-                    S.bcnt[lane] = inc - v;
+#pragma unroll
+                    for (int w = 0; w < IM_NP; ++w) S.wcnt[w][lane] = inc - run + part[w];
                 }
                 im_pbar();
-                for (uint32_t q = ptid; q < nT; q += PT) {
-                    const uint32_t k = S.tkey[q];
-                    S.tnext[S.bcnt[k & 31u] + ((k >> 8) & 0xFFFFFu)] = S.tidx[q] | (k & 0x30000000u);
+                for (uint32_t q = q_lo + lane; q < q_lo + per; q += 32) {
+                    const uint32_t k = q < q_hi ? S.tkey[q] : 0u;
+                    const uint32_t bk = q < q_hi ? (k & 31u) : 64u + lane;
+                    const uint32_t m = __match_any_sync(full_mask, bk);
+                    const uint32_t below = (uint32_t)__popc(m & ((1u << lane) - 1u));
+                    if (q < q_hi) S.tnext[S.wcnt[pwarp][bk] + below] = S.tidx[q] | (k & 0x30000000u);
+                    __syncwarp();
+                    if (q < q_hi && below == 0u) S.wcnt[pwarp][bk] += (uint32_t)__popc(m);
+                    __syncwarp();
                 }
                 // ... and pull the item's records into L2, so that the bulk copies issued once the stage is free
                 // do not wait for HBM
