@@ -37,7 +37,7 @@ FLOPS_PER_CANDIDATE, FLOPS_PER_PAIR = 8, 32      # DESIGN.md "interaction flop c
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the production interaction kernel, from
 # an `ncu --set full` capture of this command (DRAM counters cannot be read inside a timed run): config ->
 # (bytes, file under profiles/ that holds the capture).  Configs without a capture report null.
-IA_TRAFFIC = {}
+IA_TRAFFIC = {3: (3342058752 + 532709632, "ncu capture profiles/r02_opmix_config3.md (dram__bytes_read.sum + dram__bytes_write.sum)")}
 IA_KERNEL = {0: "interact_mma_kernel", 1: "interact_simple_kernel", 2: "interact_staged_kernel"}
 # algorithmic HBM bytes per particle of the memory-bound stages
 BYTES = dict(keys=28.0, sort_per_pass=16.0, gather=116.0, verlet=116.0, migrate=4.0)
@@ -197,12 +197,13 @@ def migrate_bytes(n: int, n_mig: int) -> float:
 
 def stage_entry(ms: float, nbytes, hbm_gbs: float, **extra) -> dict:
     """One HBM-bound stage: algorithmic GB/s and fraction of the measured copy peak.  A stage that moved
-    less than 1 MB (no migrants, tiny halo planes) is launch latency, not a bandwidth: null."""
+    less than 8 MB (no or few migrants, tiny halo planes: about 1 us at the copy bandwidth, less than the
+    launch latency of its kernels) is launch latency, not a bandwidth: null."""
     d = dict(ms=ms, **extra)
     if nbytes is None:
         return d
-    if nbytes < 1e6:
-        d.update(algorithmic_gbs=None, frac_of_hbm_peak=None, note="< 1 MB moved: launch latency, not a bandwidth")
+    if nbytes < 8e6:
+        d.update(algorithmic_gbs=None, frac_of_hbm_peak=None, note="< 8 MB moved: launch latency, not a bandwidth")
         return d
     gbs = nbytes / (ms * 1e-3) / 1e9
     d.update(algorithmic_gbs=gbs, frac_of_hbm_peak=gbs / hbm_gbs)
