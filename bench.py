@@ -435,7 +435,7 @@ def main():
     sm_mhz = clocks.get("sm_mhz") or pk["sm_max_mhz"]
     # the FP32 peak this box really sustains: register-resident FMA chains, same process (csrc/fma_peak.cu)
     peak_meas = max(sph.sph_fma_peak(0, 8192), sph.sph_fma_peak(1, 8192))
-    traffic, traffic_src = IA_TRAFFIC.get(args.config if not args.disorder else None, (None, None))
+    traffic, traffic_src = IA_TRAFFIC.get(args.config if not (args.disorder or args.adaptive or args.variant) else None, (None, None))
     roofline = dict(bound="alu", kernel=IA_KERNEL.get(args.variant, "?"), achieved=achieved, peak=peak, unit="TFLOP/s",
                     frac=achieved / peak, traffic=traffic, traffic_source=traffic_src,
                     peak_source=f"148 SMs x 128 FP32 lanes x 2 flop x {pk['sm_max_mhz']:.0f} MHz (max clock, {pk['source']})",
