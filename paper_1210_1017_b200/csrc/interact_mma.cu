@@ -74,6 +74,10 @@ constexpr int IM_BATCH = IM_CAP - 128;       // particles per batch (16 x 5 x 27
                                              // of 32 slots, which costs up to 4 x 31 padding slots
 constexpr int IM_RB = SPH_IM_RB;             // mask ring: blocks of 64 candidates per warp per round
 constexpr int IM_STAGES = 2;
+#ifndef SPH_IM_PPS
+#define SPH_IM_PPS 2
+#endif
+constexpr int IM_PPS = SPH_IM_PPS;           // pair slots per drain step (even): IM_PPS pops, IM_PPS / 2 packed pair terms
 constexpr float IM_WIDE_N = -3.0e38f;        // |x|^2 stand-in of "wide" tiles: every real record is a hit
 constexpr float IM_FAR = 1e15f;              // coordinate of the dummy partner: r2 = 3e30 is finite, shape = 0
 constexpr float IM_TINY = 1e-30f;            // added to r2: a coincident pair (the particle itself) adds exactly 0
@@ -746,7 +750,7 @@ __device__ __forceinline__ void im_chunk(ImStage &T, uint32_t mwarp, uint32_t ch
                 // so that no shared-memory load sits on the chain from one pop to the next
                 uint32_t cur = odd ? 1u : 0u;
                 uint32_t atop = dummy_addr;
-                const uint32_t steps = __reduce_max_sync(full_mask, tot ? (tot + odd + 3u) >> 2 : 0u);
+                const uint32_t steps = __reduce_max_sync(full_mask, tot ? (tot + odd + (uint32_t)(IM_PPS - 1)) / (uint32_t)IM_PPS : 0u);
                 odd = (odd + tot) & 1u;
                 const uint32_t atop0 = recA_addr + 16u * (rb0 * 64u + 32u * 31u + 31u);   // word k: atop0 - 512 (31 - k)
                 const uint32_t mtop = mlane + 128u * 31u;                                   // word k at mtop - 128 (31 - k)
@@ -777,12 +781,27 @@ __device__ __forceinline__ void im_chunk(ImStage &T, uint32_t mwarp, uint32_t ch
                     return lin ^ ((lin >> 3) & 0x60u);                                  // slot swizzle, in bytes
                 };
                 // software pipeline: the addresses of step st + 1 are popped before the pairs of step st are evaluated
-                uint32_t sa = pop(), sb = pop(), sc = pop(), sd = pop();
-                for (uint32_t st = 0; st < steps; ++st) {
-                    const uint32_t na = pop(), nb2 = pop(), nc = pop(), nd = pop();     // past the last hit: dummy partners
-                    pair2(sa, sb);
-                    pair2(sc, sd);
-                    sa = na; sb = nb2; sc = nc; sd = nd;
+                uint32_t cs[IM_PPS];
+#pragma unroll
+                for (int q = 0; q < IM_PPS; ++q) cs[q] = pop();
+                // two steps per iteration (independent chains for the scheduler), a single one if the count is odd
+                uint32_t st = 0;
+                for (; st + 1u < steps; st += 2u) {
+                    uint32_t n1[IM_PPS], n2[IM_PPS];                                    // past the last hit: dummy partners
+#pragma unroll
+                    for (int q = 0; q < IM_PPS; ++q) n1[q] = pop();
+#pragma unroll
+                    for (int q = 0; q < IM_PPS; ++q) n2[q] = pop();
+#pragma unroll
+                    for (int q = 0; q < IM_PPS; q += 2) pair2(cs[q], cs[q + 1]);
+#pragma unroll
+                    for (int q = 0; q < IM_PPS; q += 2) pair2(n1[q], n1[q + 1]);
+#pragma unroll
+                    for (int q = 0; q < IM_PPS; ++q) cs[q] = n2[q];
+                }
+                if (st < steps) {
+#pragma unroll
+                    for (int q = 0; q < IM_PPS; q += 2) pair2(cs[q], cs[q + 1]);
                 }
                 __syncwarp();
             }
