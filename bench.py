@@ -37,7 +37,7 @@ FLOPS_PER_CANDIDATE, FLOPS_PER_PAIR = 8, 32      # DESIGN.md "interaction flop c
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the production interaction kernel, from
 # an `ncu --set full` capture of this command (DRAM counters cannot be read inside a timed run): config ->
 # (bytes, file under profiles/ that holds the capture).  Configs without a capture report null.
-IA_TRAFFIC = {3: (3342058752 + 532709632, "ncu capture profiles/r02_opmix_config3.md (dram__bytes_read.sum + dram__bytes_write.sum)")}
+IA_TRAFFIC = {3: (3316548096 + 533717760, "ncu capture profiles/r02_opmix_config3.md (dram__bytes_read.sum + dram__bytes_write.sum)")}
 IA_KERNEL = {0: "interact_mma_kernel", 1: "interact_simple_kernel", 2: "interact_staged_kernel"}
 # algorithmic HBM bytes per particle of the memory-bound stages
 BYTES = dict(keys=28.0, sort_per_pass=16.0, gather=116.0, verlet=116.0, migrate=4.0)
