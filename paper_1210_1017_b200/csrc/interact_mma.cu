@@ -850,15 +850,9 @@ interact_mma_kernel(const float4 *__restrict__ pos4, const float4 *__restrict__ 
     __syncthreads();
 
     if (warp < IM_NP) {
-#ifdef SPH_IM_REGS_CONSUMER
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(SPH_IM_REGS_PRODUCER));   // registers go to the consumers
-#endif
         im_produce<UNIFORM>(S, pos4, velrho4, idt, cell_begin, g, ph, A);
         return;
     }
-#ifdef SPH_IM_REGS_CONSUMER
-    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(SPH_IM_REGS_CONSUMER));
-#endif
     const uint32_t mwarp = (uint32_t)__cvta_generic_to_shared(&S.mask[warp - IM_NP][0]);
     for (uint32_t it = 0;; ++it) {
         const uint32_t s = it & 1u;
