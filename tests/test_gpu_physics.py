@@ -45,6 +45,27 @@ def test_config0_rest_state_rates(variant):
 
 
 @pytest.mark.parametrize("variant", [0, 1, 2])
+def test_disordered_positions_rates(variant):
+    """No lattice: every fluid particle is moved by U(-0.3, 0.3) dp per axis (seeded), on top of random
+    velocities and densities.  Neighbour counts then differ from particle to particle (the lanes of a warp
+    drain different numbers of pairs), pairs sit anywhere around the cut-off instead of exactly at 2h, and
+    cells hold 20-35 particles instead of 27."""
+    w = W.dam_break(32, scrambled=True)
+    nf = w.n_fluid
+    ids = np.arange(nf, dtype=np.int64)
+    dp = w.params["dp"]
+    pos = w.pos.astype(np.float64)
+    for c in range(3):
+        pos[:nf, c] += (2.0 * W.u01(W.SEED_STATE + 7, ids, c) - 1.0) * 0.3 * dp
+    w.pos = pos.astype(np.float32)
+    ref_a, ref_d = oracle_rates(w)
+    out = _gpu_rates(w, variant)
+    e_d, e_a = rate_errors(w, out["acc"], out["drho"], ref_a, ref_d)
+    assert e_d <= TOL_RATE, e_d
+    assert e_a <= TOL_RATE, e_a
+
+
+@pytest.mark.parametrize("variant", [0, 1, 2])
 @pytest.mark.parametrize("nb", [16, 40])
 def test_scrambled_state_rates(variant, nb):
     """Reading A21: same positions, random velocities and densities, so that pressure,
