@@ -48,7 +48,8 @@ enum {
     SPH_ERR_CUDA = -5,            /* a CUDA runtime call failed (sticky) */
     SPH_ERR_NONFINITE = -6,       /* a non-finite position/velocity/density was seen on the
                                      device (sticky flag, reported by sph_status) */
-    SPH_ERR_ORDER = -7            /* call order violated (e.g. sph_interact before a sort) */
+    SPH_ERR_ORDER = -7,           /* call order violated (e.g. sph_interact before a sort) */
+    SPH_ERR_STATIC_LIMIT = -8     /* sph_cell_table_static: size beyond its fixed built-in scratch */
 };
 
 typedef struct sph_ctx sph_ctx;   /* opaque */
@@ -246,6 +247,46 @@ int sph_launch_count(const sph_ctx *ctx, uint64_t *out);
  * FMA lanes per thread on 148 x 8 CTAs of 256 threads; HOST *tflops = 2 flop per FMA / CUDA-event time.
  * The denominator bench.py reports beside the nominal 148 x 128 x 2 x clock.  Synchronises. */
 int sph_fma_peak(sph_ctx *ctx, int variant, int iters, double *tflops);
+
+/* The cell table without a context, a workspace or any allocation (a4: the "extra array
+ * ... with the index of the first particle of each cell"; L276 "first and last particle in a given region").
+ *
+ * Why it exists: every other call works out of the workspace the caller allocated for sph_init.  A caller
+ * that cannot allocate device memory has nothing to hand over - for instance an analysis or coupling code
+ * that was only lent the pointers of an sph_view, a plug-in in a process whose framework already owns all
+ * of the GPU's memory (a plain cudaMalloc fails there), or a loop that must not take the device-wide stall
+ * of cudaMalloc / cudaFree.  This call needs from the caller only its input and its output; the scratch it
+ * uses (a work list of long runs of empty cells, plus a counter) is an array of SPH_STATIC_SCRATCH_BYTES
+ * (about 2 MiB) built into the library, present on every GPU that loads the library until the process ends.
+ * It calls no cudaMalloc, cudaFree or allocating library routine.
+ *
+ *   keyword     DEVICE, n words, non-decreasing in bits 0..27 (the cell label; bits 28..31 are ignored) -
+ *               e.g. sph_view.keyword, or the keywords of one sub-domain's particles.  Read only.
+ *   n           number of particles, <= 2^28; n = 0 gives an all-zero table
+ *   ncells      number of cells, 1 <= ncells <= SPH_STATIC_MAX_CELLS; labels >= ncells count as ncells - 1
+ *   cell_begin  DEVICE, ncells + 1 words, written in full: cell_begin[c] = number of particles whose cell
+ *               label is below c (index of the first particle of cell c; cell_begin[ncells] = n) - the
+ *               same values sph_sort_and_cells leaves in sph_view.cell_begin
+ *   cuda_stream cudaStream_t as void*, NULL = legacy default stream; work is enqueued, not waited for
+ *
+ * Limits and rules, all consequences of the scratch being one fixed array:
+ *   - ncells > SPH_STATIC_MAX_CELLS (or n > 2^28) is refused with SPH_ERR_STATIC_LIMIT and nothing is
+ *     launched; use sph_sort_and_cells with a workspace for larger grids.
+ *   - All calls on one GPU share the array, from every thread and stream of the process.  Two calls whose
+ *     GPU work may overlap (different streams without an ordering between them) race on it and give wrong
+ *     tables; order them on one stream or with events.  The array keeps the previous call's contents; the
+ *     call itself resets the one word that has to start at zero.
+ *   - The first call on each GPU looks up where that GPU's copy of the array lives (cudaGetSymbolAddress,
+ *     done with the calling thread's current device, result kept).  Make that first call during set-up,
+ *     before any stream capture begins.  The device that is current at the call must be the one that owns
+ *     keyword, cell_begin and the stream.
+ * Returns SPH_OK or SPH_ERR_ARG / SPH_ERR_STATIC_LIMIT / SPH_ERR_CUDA; sph_cell_table_static_error() is the
+ * text of the calling thread's last failure of this call ("" if it succeeded). */
+#define SPH_STATIC_MAX_CELLS (1u << 22)
+#define SPH_STATIC_SCRATCH_BYTES 2098560u
+int sph_cell_table_static(const uint32_t *keyword, uint64_t n, uint32_t ncells, uint32_t *cell_begin,
+                          void *cuda_stream);
+const char *sph_cell_table_static_error(void);
 
 void sph_destroy(sph_ctx *ctx);
 const char *sph_strerror(int code);

@@ -32,7 +32,11 @@ EXPORTS = ["sph_workspace_bytes", "sph_init", "sph_set_state", "sph_set_slabs", 
            "sph_sort_and_cells", "sph_build_halos", "sph_interact", "sph_interact_slab", "sph_step", "sph_time_step", "sph_step_adaptive", "sph_get_view",
            "sph_download", "sph_status", "sph_set_option", "sph_profile_enable", "sph_profile_read",
            "sph_pair_stats", "sph_launch_count", "sph_destroy", "sph_strerror", "sph_balance_slabs",
-           "sph_download_resume", "sph_set_resume", "sph_last_cuda_error", "sph_fma_peak"]
+           "sph_download_resume", "sph_set_resume", "sph_last_cuda_error", "sph_fma_peak",
+           "sph_cell_table_static", "sph_cell_table_static_error"]
+SPH_ERR_STATIC_LIMIT = -8
+SPH_STATIC_MAX_CELLS = 1 << 22
+SPH_STATIC_SCRATCH_BYTES = 2098560
 
 
 class sph_params(C.Structure):
@@ -107,6 +111,10 @@ _lib.sph_last_cuda_error.restype = C.c_char_p
 _lib.sph_last_cuda_error.argtypes = [C.c_void_p]
 _lib.sph_fma_peak.restype = C.c_int
 _lib.sph_fma_peak.argtypes = [C.c_void_p, C.c_int, C.c_int, C.POINTER(C.c_double)]
+_lib.sph_cell_table_static.restype = C.c_int
+_lib.sph_cell_table_static.argtypes = [C.c_void_p, C.c_uint64, C.c_uint32, C.c_void_p, C.c_void_p]
+_lib.sph_cell_table_static_error.restype = C.c_char_p
+_lib.sph_cell_table_static_error.argtypes = []
 _lib.sph_destroy.restype = None
 _lib.sph_destroy.argtypes = [C.c_void_p]
 _lib.sph_strerror.restype = C.c_char_p
@@ -126,6 +134,27 @@ def sph_strerror(code: int) -> str:
 def _check(rc: int) -> None:
     if rc != SPH_OK:
         raise SphError(rc)
+
+
+def sph_cell_table_static(keyword, ncells: int, cell_begin, stream=None) -> None:
+    """Cell table of a sorted keyword array for callers that cannot allocate device memory (they hold
+    only borrowed pointers, or their process has no free GPU memory left to ask for): the scratch is a
+    fixed array inside the library, so ncells is limited to SPH_STATIC_MAX_CELLS and calls on one GPU must
+    not overlap.  keyword: int32 CUDA tensor of n sorted keywords (e.g. view_tensors()["keyword"]);
+    cell_begin: int32 CUDA tensor of ncells + 1 entries on the same device, written in full.  The call is
+    enqueued on ``stream`` (default: torch's current stream of that device).  See include/sph_b200.h."""
+    import torch
+    assert keyword.is_cuda and cell_begin.is_cuda and keyword.device == cell_begin.device
+    assert keyword.dtype == torch.int32 and cell_begin.dtype == torch.int32
+    assert keyword.is_contiguous() and cell_begin.is_contiguous()
+    assert cell_begin.numel() == int(ncells) + 1
+    with torch.cuda.device(keyword.device):
+        st = stream if stream is not None else torch.cuda.current_stream(keyword.device)
+        rc = _lib.sph_cell_table_static(C.c_void_p(keyword.data_ptr() if keyword.numel() else None),
+                                        int(keyword.numel()), int(ncells), C.c_void_p(cell_begin.data_ptr()),
+                                        C.c_void_p(st.cuda_stream))
+    if rc != SPH_OK:
+        raise SphError(rc, _lib.sph_cell_table_static_error().decode())
 
 
 def make_params(P: dict) -> sph_params:

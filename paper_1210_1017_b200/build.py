@@ -16,7 +16,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libsph_b200.so")
 SOURCES = ["sph_api.cu", "keys.cu", "radix_sort.cu", "gather_cells.cu", "halo_migrate.cu",
-           "interact.cu", "interact_mma.cu", "verlet.cu", "slab_exec.cu", "fma_peak.cu"]
+           "interact.cu", "interact_mma.cu", "verlet.cu", "slab_exec.cu", "fma_peak.cu", "cell_table_static.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-I", os.path.join(ROOT, "include"), "-I", CSRC]
 

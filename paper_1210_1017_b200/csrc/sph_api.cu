@@ -773,6 +773,7 @@ const char *sph_strerror(int code)
     case SPH_ERR_CUDA: return "CUDA runtime error";
     case SPH_ERR_NONFINITE: return "non-finite particle state on the device";
     case SPH_ERR_ORDER: return "call order violated (sort first)";
+    case SPH_ERR_STATIC_LIMIT: return "size beyond the built-in scratch of sph_cell_table_static";
     default: return "unknown error";
     }
 }

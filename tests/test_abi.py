@@ -67,7 +67,7 @@ def test_workspace_bytes_and_argument_errors(B):
     assert B._lib.sph_init(C.byref(ctx), C.byref(bad), C.byref(part), 1, None, 0, None) == -1
     assert B._lib.sph_init(C.byref(ctx), C.byref(B.make_params(big)), C.byref(part), 1, None, 0, None) == -3
     assert B.sph_strerror(0) == "ok" and "slab" in B.sph_strerror(-4)
-    for code in range(-7, 1):
+    for code in range(-8, 1):
         assert B.sph_strerror(code) != "unknown error"
 
 
