@@ -193,8 +193,9 @@ def uniform_cube(n: int, seed: int = SEED_POS, n_slabs: int = 8, chunk: int = 1 
     """n particles uniform in [0,1)^3, ids in generation order (random cell keys), cell
     size 2h with a mean of ~30 neighbours inside the 2h sphere, velocities U(-1,1).
 
-    ``prev_slab`` is a synthetic previous owner: the k/S-slab of x shifted left by
-    U(0,0.2)*2h, so a few per cent of the particles show up as migrants.
+    ``prev_slab`` is a synthetic previous owner: the k/S-slab of x shifted by U(-0.2,0.2)*2h,
+    so a few per cent of the particles show up as migrants, about half of them in each direction
+    (labels 1 and 2 of PAPER.md L264).
     """
     two_h = (90.0 / (4.0 * math.pi * n)) ** (1.0 / 3.0)
     h = 0.5 * two_h
@@ -208,7 +209,7 @@ def uniform_cube(n: int, seed: int = SEED_POS, n_slabs: int = 8, chunk: int = 1 
             pos[a:b, c] = u01(seed, ids, c).astype(np.float32)
         for c in range(3):
             vel[a:b, c] = (2.0 * u01(SEED_STATE, ids, c) - 1.0).astype(np.float32)
-        xs = pos[a:b, 0].astype(np.float64) - 0.2 * two_h * u01(SEED_STATE, ids, 3)
+        xs = pos[a:b, 0].astype(np.float64) + 0.2 * two_h * (2.0 * u01(SEED_STATE, ids, 3) - 1.0)
         prev[a:b] = np.clip(np.floor(xs * n_slabs), 0, n_slabs - 1).astype(np.uint8)
     # fp32 rounding can push u < 1 up to exactly 1.0f; keep the cube half-open
     np.minimum(pos, np.float32(np.nextafter(np.float32(1.0), np.float32(0.0))), out=pos)

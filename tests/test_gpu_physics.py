@@ -222,3 +222,38 @@ def test_config1_full_size_sampled_rates():
         scale_a = max(scale_a, np.abs(a[k]).max())
         scale_d = max(scale_d, abs(d[k]))
     assert worst_a <= TOL_RATE * scale_a and worst_d <= TOL_RATE * scale_d
+
+
+def test_moving_wall_particles_are_not_integrated_but_act_on_the_fluid():
+    """boundary particles obey the same equations as the fluid, but "the integration update for
+    position and velocity is not performed" (their motion is "externally imposed").  The wall particles of a
+    dam break are given a velocity: after sph_step their r and v must keep their bits while their density
+    moves; the fluid next to them must feel the wall's velocity (its d rho/dt differs from the static-wall
+    value) and still match ORACLE B to the one-step tolerance."""
+    w = W.dam_break(16, scrambled=True)
+    bd = w.type == 1
+    ids = np.arange(w.n, dtype=np.int64)
+    w_static_d = oracle_rates(w)[1]
+    for c in range(3):
+        w.vel[bd, c] = ((2.0 * W.u01(W.SEED_STATE + 11, ids[bd], c) - 1.0) * 0.5).astype(np.float32)
+    ref_a, ref_d = oracle_rates(w)
+    fl = ~bd
+    assert np.abs(ref_d[fl] - w_static_d[fl]).max() > 1e-2 * np.abs(ref_d).max()
+    sph = make_sph(w)
+    sph.sph_sort_and_cells()
+    sph.sph_interact()
+    out = sph.sph_download()
+    e_d, e_a = rate_errors(w, out["acc"], out["drho"], ref_a, ref_d)
+    assert e_d <= TOL_RATE and e_a <= TOL_RATE, (e_d, e_a)
+    s = OB.State(w.pos, w.vel, w.rho, w.type)
+    p = OB.params_from_workload(w.params)
+    for _ in range(3):
+        sph.sph_step(w.dt)
+        OB.step(p, s, w.dt, verlet_ns=w.params["verlet_ns"])
+    out = sph.sph_download(acc=False, drho=False)
+    assert sph.sph_status() == 0
+    assert np.array_equal(out["pos"][bd].view(np.uint32), w.pos[bd].view(np.uint32))      # bit-unchanged
+    assert np.array_equal(out["vel"][bd].view(np.uint32), w.vel[bd].view(np.uint32))
+    assert (out["rho"][bd] != w.rho[bd]).mean() > 0.5
+    assert rel_l2(out["rho"][bd] - w.rho[bd].astype(np.float64), s.rho[bd] - w.rho[bd]) <= 1e-2
+    assert rel_l2(out["rho"], s.rho) <= TOL_STATE and rel_l2(out["vel"][fl], s.v[fl]) <= TOL_STATE

@@ -221,8 +221,9 @@ def test_cell_list_equals_brute_force_bitwise():
 def test_verlet_free_fall_and_fixed_boundary():
     g = 9.81
     p = OB.make_params(h=0.1, g=(0, 0, -g))
-    # two far-apart particles: one fluid, one boundary
-    s = OB.State([[0, 0, 10.0], [50, 0, 0]], [[0.3, 0, 0], [0, 0, 0]], [1000, 1000], [0, 1])
+    # two far-apart particles: one fluid, one boundary.  The boundary particle CARRIES a velocity (an
+    # "externally imposed" one, L116): integrating it would move it, so the branch is visible
+    s = OB.State([[0, 0, 10.0], [50, 0, 0]], [[0.3, 0, 0], [0.2, 0, 0]], [1000, 1000], [0, 1])
     dt, ns = 1e-3, 4
     for n in range(1, 11):                       # exercises corrective (n % 4 == 0) and leapfrog steps
         OB.step(p, s, dt, verlet_ns=ns, mode=0)
@@ -230,8 +231,39 @@ def test_verlet_free_fall_and_fixed_boundary():
         assert abs(s.r[0, 2] - (10.0 - 0.5 * g * t * t)) < 1e-12
         assert abs(s.v[0, 2] + g * t) < 1e-12
         assert abs(s.r[0, 0] - 0.3 * t) < 1e-12
-        assert (s.r[1] == [50, 0, 0]).all() and (s.v[1] == 0).all()
+        # L116: "the integration update for position and velocity is not performed"
+        assert (s.r[1] == [50, 0, 0]).all() and (s.v[1] == [0.2, 0, 0]).all()
     assert s.rho[0] == 1000 and s.rho[1] == 1000
+
+
+def test_boundary_particle_density_evolves_but_position_and_velocity_do_not():
+    """boundary particles "satisfy the same equations as the fluid particles" except that
+    "the integration update for position and velocity is not performed" - so next to approaching fluid a
+    moving wall particle's density follows its continuity rate (Eq. 7) while r and v keep their bits.
+    The rate is pinned by hand: d rho_b/dt = m_f (v_b - v_f) . grad_b W(r_b - r_f), Wendland C2 in 3-D,
+    dW/dr = -(105 / (16 pi h^5)) r (1 - r/2h)^3  (written out here, not taken from the oracle)."""
+    h, m = 0.1, 0.7
+    p = OB.make_params(h=h, g=(0, 0, -9.81), mass_fluid=m, mass_bound=m)
+    rb, rf = np.array([0.0, 0.0, 0.0]), np.array([0.12, 0.0, 0.05])
+    vb, vf = np.array([0.2, -0.1, 0.0]), np.array([-1.0, 0.0, 0.5])
+    s = OB.State([rb, rf], [vb, vf], [1000.0, 1000.0], [1, 0])
+    d = rb - rf
+    r = float(np.linalg.norm(d))
+    dWdr = -(105.0 / (16.0 * np.pi * h ** 5)) * r * (1.0 - r / (2 * h)) ** 3
+    drho_b = m * float(np.dot(vb - vf, d / r)) * dWdr
+    assert abs(drho_b) > 1.0
+    dt = 1e-4
+    rho = [1000.0]
+    for n in range(3):                           # step 0 is one-sided, steps 1, 2 use rho_m1 + 2 dt rate
+        rates_a, rates_d = OB.rates(p, s.r, s.v, s.rho, s.type, mode=0)
+        if n == 0:
+            assert abs(rates_d[0] - drho_b) <= 1e-12 * abs(drho_b)
+        assert (rates_a[0] == 0).all()           # no acceleration is kept for a boundary particle
+        rho.append((rho[-1] if n == 0 else rho[-2]) + (1 if n == 0 else 2) * dt * rates_d[0])
+        OB.step(p, s, dt, verlet_ns=40, mode=0)
+        assert (s.r[0] == rb).all() and (s.v[0] == vb).all()            # bit-unchanged
+        assert abs(s.rho[0] - rho[-1]) <= 1e-12 * 1000.0 and s.rho[0] != 1000.0
+        assert (s.r[1] != rf).any() and (s.v[1] != vf).any()            # the fluid particle does move
 
 
 def test_verlet_uses_two_step_form_between_corrections():

@@ -156,6 +156,32 @@ def test_structure_vs_brute_force():
     assert A["mig_count"].sum() == len(m) > 0
 
 
+def test_migration_labels_both_directions_by_hand():
+    """"particles are labeled as '1' if they migrated to left, '2' if they migrated to right,
+    and '0' if they stayed"; L240: the same 1 / 2 / 0 for left edge / right edge / interior.  Six particles
+    on a 6 x 1 x 1 grid (cell side 2h = 1, x = cell + 0.5 exactly), planes 0|2|4|6, previous owners chosen
+    so that two moved left, two moved right and two stayed.  Every expected value below is written by
+    hand from those two sentences and the keyword layout of include/sph_b200.h (cell in bits 0..27, edge
+    label in bits 28..29, migration label in bits 30..31)."""
+    pos = np.array([[k + 0.5, 0.5, 0.5] for k in range(6)], dtype=np.float32)
+    planes = [0, 2, 4, 6]
+    #                 id: 0  1  2  3  4  5        owner now: 0 0 1 1 2 2
+    prev = np.array([1, 0, 2, 0, 1, 2], dtype=np.uint8)   # 0: 1->0 left, 2: 2->1 left, 3: 0->1 right, 4: 1->2 right
+    slab = np.array([0, 0, 1, 1, 2, 2])
+    assert list(OA.mig_label(slab, prev)) == [1, 0, 1, 2, 2, 0]
+    assert list(OA.mig_label(slab, None)) == [0] * 6
+    assert list(OA.halo_label(np.arange(6), planes)) == [0, 2, 1, 2, 1, 0]
+    A = OA.structure(pos, np.arange(6), (0.0, 0.0, 0.0), (6.0, 1.0, 1.0), 0.5, planes, prev)
+    assert tuple(A["nc"]) == (6, 1, 1)
+    assert [int(k) for k in A["keyword_sorted"]] == [0x40000000, 0x20000001, 0x50000002, 0xA0000003,
+                                                     0x90000004, 0x00000005]
+    assert [tuple(int(x) for x in row) for row in A["migrants"]] == [(0, 0, 1, 0), (2, 2, 2, 1), (3, 3, 0, 1),
+                                                                     (4, 4, 1, 2)]
+    # mig_count[s] = (left slab s towards the left, towards the right): 3 left slab 0 rightwards; 0 and 4
+    # left slab 1 (one each way); 2 left slab 2 leftwards
+    assert A["mig_count"].tolist() == [[0, 1], [1, 1], [1, 0]]
+
+
 def test_halo_sufficiency_against_brute_force_neighbours():
     """Every neighbour (0 < r < 2h) of a particle owned by slab s is owned by s or is in
     the halo L_s u R_s (halo width = interaction range 2h)."""
