@@ -40,7 +40,8 @@ FLOPS_PER_CANDIDATE, FLOPS_PER_PAIR = 8, 32      # DESIGN.md "interaction flop c
 IA_TRAFFIC = {3: (3316548096 + 533717760, "ncu capture profiles/r02_opmix_config3.md (dram__bytes_read.sum + dram__bytes_write.sum)")}
 IA_KERNEL = {0: "interact_mma_kernel", 1: "interact_simple_kernel", 2: "interact_staged_kernel"}
 # algorithmic HBM bytes per particle of the memory-bound stages
-BYTES = dict(keys=28.0, sort_per_pass=16.0, gather=116.0, verlet=116.0, migrate=4.0)
+# dt_reduce (sph_time_step): acc4 16 + velrho4 16 + mumax 4 + idt 4 B read per particle
+BYTES = dict(keys=28.0, sort_per_pass=16.0, gather=116.0, verlet=116.0, migrate=4.0, dt_reduce=40.0)
 
 
 def peaks():
@@ -212,13 +213,22 @@ def stage_entry(ms: float, nbytes, hbm_gbs: float, **extra) -> dict:
 
 def run_micro(args):
     """Sort/halo microbenchmark (configs[4]); prints its own JSON (not the driver's line)."""
+    print(json.dumps(micro_measure(args.micro, args.steps, args.warmup,
+                                   cpu_baseline=not args.no_cpu_baseline and args.micro <= 26)))
+
+
+def micro_measure(log2n: int, steps: int, warmup: int, cpu_baseline: bool, device: str = "cuda:0") -> dict:
+    """BASELINE.json configs[4] at N = 2^log2n: uniform-random positions, 8 logical x-slabs, synthetic previous
+    owners; every iteration restores the random order (untimed) and times sph_sort_and_cells + sph_build_halos
+    with the stage timers.  Returns Gkeys/s and the HBM fraction of every stage."""
     import torch
     from paper_1210_1017_b200 import binding as B
     from paper_1210_1017_b200 import workloads as W
+    args = argparse.Namespace(steps=steps, warmup=warmup, micro=log2n, no_cpu_baseline=not cpu_baseline)
     n = 1 << args.micro
     w = W.uniform_cube(n)
     pk = peaks()
-    sph = B.Sph(w.params, w.pos, w.vel, w.rho, w.type, prev_slab=w.prev_slab)
+    sph = B.Sph(w.params, w.pos, w.vel, w.rho, w.type, prev_slab=w.prev_slab, device=device)
     v = sph.sph_get_view()
     planes = W.slab_planes(v.nc[0], 8)
     sph.sph_set_slabs(planes)
@@ -262,7 +272,9 @@ def run_micro(args):
     gc_ms = med["gather"] + med["cells"]
     gc_b = byts["gather"] + 4.0 * (v.ncells + 1)
     out["stages"]["gather+cells"] = stage_entry(gc_ms, gc_b, pk["hbm_gbs"])
-    print(json.dumps(out))
+    out["iterations"] = dict(timed=reps, warmup=args.warmup, figure="median over the timed iterations")
+    sph.sph_destroy()
+    return out
 
 
 def main():
@@ -278,6 +290,9 @@ def main():
     ap.add_argument("--cpu-sample", type=int, default=1_500_000, help="particles of the cpu_baseline sample")
     ap.add_argument("--ref-sample", type=int, default=300_000, help="particles per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--main-micro", type=int, default=26, metavar="LOG2N",
+                    help="after the main measurement (config 3, N = 1 only), run the sort/halo microbenchmark at 2^LOG2N "
+                         "in the same process and attach it to the JSON line under 'micro' (0 = skip)")
     ap.add_argument("--variant", type=int, default=0)
     ap.add_argument("--disorder", type=int, default=0, metavar="K",
                     help="time a DISORDERED fluid instead of the rest-state lattice: scrambled start (random "
@@ -450,7 +465,7 @@ def main():
     n_mig = int(T["mig_total"].item())
     byts = dict(keys=BYTES["keys"] * n, sort=BYTES["sort_per_pass"] * passes * n, gather=BYTES["gather"] * n,
                 cells=None, halo=72.0 * n_halo, migrate=migrate_bytes(n, n_mig),
-                verlet=BYTES["verlet"] * n)
+                verlet=BYTES["verlet"] * n, dt_reduce=BYTES["dt_reduce"] * n)
     stages = {}
     for k, (ms, c) in stage.items():
         if c == 0:
@@ -464,6 +479,17 @@ def main():
         ks_ms = stages["keys"]["ms"] + stages["sort"]["ms"]
         stages["keys+sort"] = stage_entry(ks_ms, byts["keys"] + byts["sort"], pk["hbm_gbs"],
                                           share=ks_ms * args.steps / ms_total)
+    # ---- BASELINE.json configs[4] on the same line: the >= 60 % HBM bars of the sort and compaction kernels
+    # are quoted on the random-order microbenchmark, not on the (nearly sorted) simulation state
+    micro = None
+    if args.main_micro and world == 1 and args.config == 3 and not (args.adaptive or args.disorder or args.variant):
+        sph.sph_destroy()
+        del sph, T, pin, outp
+        torch.cuda.empty_cache()
+        try:
+            micro = micro_measure(args.main_micro, 5, 3, cpu_baseline=False, device=f"cuda:{local}")
+        except Exception as ex:                                  # the main figures stand on their own
+            micro = dict(error=f"{type(ex).__name__}: {ex}")
     cpu = None
     if not args.no_cpu_baseline:
         oracle_step_sample(w, 20_000)                         # builds / warms the oracle library
@@ -486,7 +512,7 @@ def main():
                     if n > 5_000_000 else "working set fits L2 (small config)"),
         clocks=clocks, e2e=e2e, gpu_launches=int(launches), roofline=roofline, cpu_baseline=cpu,
         sort_gkeys_s=n / (stages["sort"]["ms"] * 1e-3) / 1e9 if "sort" in stages else None,
-        stages=stages, hbm_peak_gbs=pk["hbm_gbs"], peak_source=pk["source"])
+        stages=stages, micro=micro, hbm_peak_gbs=pk["hbm_gbs"], peak_source=pk["source"])
     print(json.dumps(line))
     R.finalize(rep)
 

@@ -110,12 +110,14 @@ typedef struct {
     const uint32_t *migrants;     /* mig_total uint4 records (id, sortedIndex, prevSlab, slab),
                                      in sorted order */
     const uint32_t *mig_count;    /* n_slabs*2: particles that left slab s to the left / right */
+    const float *mumax;           /* n: max_j |mu_ij| of every particle over its neighbours (L112, L150), sorted
+                                     order; valid after an sph_interact made with SPH_OPT_ADAPTIVE_DT = 1 */
 } sph_view;
 
 /* Stage timers (sph_profile_*): indices into the ms[] array. */
 enum {
     SPH_T_KEYS = 0, SPH_T_SORT, SPH_T_GATHER, SPH_T_CELLS, SPH_T_HALO, SPH_T_MIGRATE,
-    SPH_T_INTERACT, SPH_T_VERLET, SPH_T_COUNT
+    SPH_T_INTERACT, SPH_T_VERLET, SPH_T_DTREDUCE /* the reduction kernel of sph_time_step */, SPH_T_COUNT
 };
 
 /* Options for sph_set_option. */
@@ -163,8 +165,10 @@ int sph_interact(sph_ctx *ctx);
  * rates of the particles slab `slab` owns, computed from its own particles and the two HALO BUFFERS
  * that sph_build_halos filled, and from nothing else - the local set is assembled, its cell table is
  * rebuilt from the particles' positions, and the production interaction kernel runs on it.  Results go
- * to the slab's range of acc4; calling it for every slab reproduces sph_interact value for value (the
- * device-side proof that a 2h halo suffices).  Needs sph_build_halos since the last sort (else
+ * to the slab's range of acc4; calling it for every slab reproduces sph_interact (the device-side proof
+ * that a 2h halo suffices): value for value while every tile next to a slab plane fits one candidate batch of
+ * the kernel (particles on or near their lattice), else to rounding, because an over-full tile is cut into
+ * batches at different candidates in the two runs and its partial sums are added in a different order.  Needs sph_build_halos since the last sort (else
  * SPH_ERR_ORDER); uses the idle halves of the state buffers as scratch; synchronises the stream once
  * (the slab ranges cross to the host). */
 int sph_interact_slab(sph_ctx *ctx, int slab);
@@ -213,8 +217,13 @@ int sph_download(sph_ctx *ctx, float *pos, float *vel, float *rho, float *acc, f
  * Verlet n-1 velocity and density (reading A7) in ID order, HOST vel_m1 n*3 and rho_m1 n (may be NULL),
  * and the number of completed steps.  To resume: sph_init / sph_set_state with the saved pos, vel, rho,
  * then sph_set_resume (HOST or DEVICE arrays, on_device says which) BEFORE the next sort (else
- * SPH_ERR_ORDER); the run then continues bit for bit as if it had never stopped (the sort order is
- * history-free, reading A12).  Both synchronise the stream (sph_set_resume only for HOST inputs). */
+ * SPH_ERR_ORDER); the particle state then continues bit for bit as if the run had never stopped (the sort
+ * order is history-free, reading A12).  One thing is NOT part of the checkpoint: the previous owner
+ * sub-domain of every particle.  The first sort after a resume therefore labels no migrants (mig_total and
+ * mig_count are 0 for that step, as after any sph_init without prev_slab) where the uninterrupted run
+ * reports the particles that crossed a plane in that step; from the second step on the migrant records
+ * agree again.  A caller that needs them across the restart passes the owners through
+ * sph_particles.prev_slab.  Both synchronise the stream (sph_set_resume only for HOST inputs). */
 int sph_download_resume(sph_ctx *ctx, float *vel_m1, float *rho_m1, uint64_t *step_index);
 int sph_set_resume(sph_ctx *ctx, const float *vel_m1, const float *rho_m1, uint64_t step_index, int on_device);
 
@@ -244,7 +253,7 @@ int sph_launch_count(const sph_ctx *ctx, uint64_t *out);
 
 /* Measured FP32 peak of this GPU: a register-resident chain of fused multiply-adds,
  * variant 0 = scalar FFMA, 1 = packed FFMA2 (two fp32 lanes per instruction); iters >= 1 rounds of 64
- * FMA lanes per thread on 148 x 8 CTAs of 256 threads; HOST *tflops = 2 flop per FMA / CUDA-event time.
+ * FMA lanes per thread on 8 CTAs of 256 threads per SM (148 x 8 on a B200); HOST *tflops = 2 flop per FMA / CUDA-event time.
  * The denominator bench.py reports beside the nominal 148 x 128 x 2 x clock.  Synchronises. */
 int sph_fma_peak(sph_ctx *ctx, int variant, int iters, double *tflops);
 

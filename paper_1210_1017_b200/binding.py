@@ -23,8 +23,8 @@ _lib = C.CDLL(LIB_PATH)
 SPH_MAX_SLABS = 16
 SPH_OK = 0
 (SPH_T_KEYS, SPH_T_SORT, SPH_T_GATHER, SPH_T_CELLS, SPH_T_HALO, SPH_T_MIGRATE, SPH_T_INTERACT,
- SPH_T_VERLET, SPH_T_COUNT) = range(9)
-STAGE_NAMES = ["keys", "sort", "gather", "cells", "halo", "migrate", "interact", "verlet"]
+ SPH_T_VERLET, SPH_T_DTREDUCE, SPH_T_COUNT) = range(10)
+STAGE_NAMES = ["keys", "sort", "gather", "cells", "halo", "migrate", "interact", "verlet", "dt_reduce"]
 SPH_OPT_INTERACT_VARIANT = 0
 SPH_OPT_ADAPTIVE_DT = 1
 
@@ -59,7 +59,7 @@ class sph_view(C.Structure):
                 ("idt", C.c_void_p), ("keyword", C.c_void_p), ("cell_begin", C.c_void_p),
                 ("slab_begin", C.c_void_p), ("halo_offset", C.c_void_p), ("halo_pos4", C.c_void_p),
                 ("halo_velrho4", C.c_void_p), ("halo_idt", C.c_void_p), ("mig_total", C.c_void_p),
-                ("migrants", C.c_void_p), ("mig_count", C.c_void_p)]
+                ("migrants", C.c_void_p), ("mig_count", C.c_void_p), ("mumax", C.c_void_p)]
 
 
 _lib.sph_workspace_bytes.restype = C.c_size_t
@@ -393,7 +393,8 @@ class Sph:
                  slab_begin=self._wrap(v.slab_begin, S + 1, i32),
                  halo_offset=self._wrap(v.halo_offset, 2 * S + 1, i32),
                  mig_total=self._wrap(v.mig_total, 1, i32),
-                 mig_count=self._wrap(v.mig_count, 2 * S, i32).view(S, 2))
+                 mig_count=self._wrap(v.mig_count, 2 * S, i32).view(S, 2),
+                 mumax=self._wrap(v.mumax, n, torch.float32))
         self.torch.cuda.current_stream(self.device).synchronize()
         self.stream.synchronize()
         nh = int(d["halo_offset"][-1].item()) if S > 1 else 0

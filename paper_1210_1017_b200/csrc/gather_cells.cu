@@ -101,7 +101,7 @@ cudaError_t launch_gather_cells(sph_ctx *c)
 // long gaps of the cell table (work list written by gather_kernel)
 cudaError_t launch_gap_fill(sph_ctx *c, uint32_t *table)
 {
-    gap_fill_kernel<<<NUM_SMS * 4, 256, 0, c->stream>>>(c->gap_list, c->counters + 8, table);
+    gap_fill_kernel<<<c->num_sms * 4, 256, 0, c->stream>>>(c->gap_list, c->counters + 8, table);
     c->n_launches++;
     return cudaGetLastError();
 }

@@ -32,8 +32,10 @@
 //    pair term in fp32, two pairs per instruction with the packed FFMA2/FMUL2/FADD2 forms of sm_100a
 //    (fma.rn.f32x2): the kernel is bound by instruction issue, not by the FP32 pipes.  Hits are consumed
 //    in groups of four; the k-th hit of a target always lands in sub-lane k & 1, so the summation order
-//    of a target depends only on its own hit sequence (per-sub-domain execution reproduces the global
-//    pass bit for bit, slab_exec.cu).
+//    of a target depends only on its own hit sequence inside a candidate batch (per-sub-domain execution,
+//    slab_exec.cu, reproduces the global pass bit for bit as long as the tiles at a slab plane need one
+//    batch; the batch cuts of an over-full tile depend on rows the slab run does not hold, and the two
+//    runs then agree to rounding only).
 //  * Tiles with more candidates than a stage holds, or more targets than its target list, are split into
 //    several ITEMS (target range x candidate batch); the items of a batch after the first ADD to the
 //    rates already written (the producer publishes them only after the previous item has drained).
@@ -196,10 +198,25 @@ __device__ __forceinline__ bool mbar_try(uint32_t mbar, uint32_t parity)
                  : "=r"(done) : "r"(mbar), "r"(parity) : "memory");
     return done != 0u;
 }
-// waiting warps sleep between polls so that they do not take issue slots from the working ones
+// waiting warps must not take issue slots from the working ones.  SPH_IM_SUSPEND_NS > 0: the wait is left to
+// the hardware - try_wait with a suspend-time hint parks the warp until the phase completes or the hint
+// runs out, so a long wait costs a handful of instructions; 0: poll and sleep SPH_IM_SLEEP_NS in between.
+#ifndef SPH_IM_SUSPEND_NS
+#define SPH_IM_SUSPEND_NS 0
+#endif
 __device__ __forceinline__ void mbar_wait(uint32_t mbar, uint32_t parity)
 {
+#if SPH_IM_SUSPEND_NS > 0
+    asm volatile("{\n\t.reg .pred p;\n\t"
+                 "IM_WAIT_%=:\n\t"
+                 "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n\t"
+                 "@p bra IM_DONE_%=;\n\t"
+                 "bra IM_WAIT_%=;\n\t"
+                 "IM_DONE_%=:\n\t}"
+                 ::"r"(mbar), "r"(parity), "r"((uint32_t)SPH_IM_SUSPEND_NS) : "memory");
+#else
     while (!mbar_try(mbar, parity)) __nanosleep(SPH_IM_SLEEP_NS);
+#endif
 }
 // 1-D bulk asynchronous copy global -> shared (SASS: UBLKCP); bytes % 16 == 0, both sides 16-byte aligned
 __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t mbar)
@@ -918,7 +935,7 @@ static cudaError_t launch_mma(sph_ctx *c)
     c->n_launches++;
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
-    const uint32_t grid = (uint32_t)(tiles < (uint64_t)NUM_SMS ? tiles : (uint64_t)NUM_SMS);
+    const uint32_t grid = (uint32_t)(tiles < (uint64_t)c->num_sms ? tiles : (uint64_t)c->num_sms);
     kern<<<grid, IM_THREADS, sizeof(ImSmem), c->stream>>>(
         ov.on ? ov.pos4 : c->pos4[c->cur], ov.on ? ov.velrho4 : c->velrho4[c->cur], ov.on ? ov.idt : c->idt[c->cur],
         cb, ov.on ? ov.acc4 : c->acc4, c->mumax, c->grid, c->phys, A);

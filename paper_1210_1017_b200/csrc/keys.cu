@@ -174,6 +174,23 @@ keys_kernel(uint32_t n, const float4 *__restrict__ pos4, const uint32_t *__restr
     }
 }
 
+// Resident CTAs per SM of the key kernel this context uses: constant per context, asked once (sph_init)
+// instead of on every step.
+cudaError_t configure_keys(sph_ctx *c)
+{
+    int per_sm = 0;
+    cudaError_t e;
+    auto occ = [&](auto kern) { return cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, 256, 0); };
+    switch (c->passes) {
+    case 1: e = occ(keys_kernel<1>); break;
+    case 2: e = occ(keys_kernel<2>); break;
+    case 3: e = occ(keys_kernel<3>); break;
+    default: e = occ(keys_kernel<4>); break;
+    }
+    c->keys_blocks_per_sm = per_sm > 0 ? per_sm : 1;
+    return e;
+}
+
 cudaError_t launch_keys(sph_ctx *c)
 {
     uint32_t n = (uint32_t)c->n;
@@ -183,16 +200,7 @@ cudaError_t launch_keys(sph_ctx *c)
     int prev_mode = c->have_prev_init ? 2 : (c->have_prev_ranges ? 1 : 0);
     uint32_t blocks = (n + 256 * KEYS_IPT - 1) / (256 * KEYS_IPT);
     // grid-stride loop: exactly one resident wave, so that no SM waits for a second, partial one
-    int per_sm = 0;
-    auto occ = [&](auto kern) { return cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, 256, 0); };
-    switch (c->passes) {
-    case 1: e = occ(keys_kernel<1>); break;
-    case 2: e = occ(keys_kernel<2>); break;
-    case 3: e = occ(keys_kernel<3>); break;
-    default: e = occ(keys_kernel<4>); break;
-    }
-    if (e != cudaSuccess) return e;
-    uint32_t cap = NUM_SMS * (uint32_t)(per_sm > 0 ? per_sm : 1);
+    uint32_t cap = (uint32_t)c->num_sms * (uint32_t)c->keys_blocks_per_sm;
     if (blocks > cap) blocks = cap;
     const float4 *pos4 = c->pos4[c->cur];
     const uint32_t *idt = c->idt[c->cur];

@@ -8,8 +8,9 @@
 // from the HALO BUFFERS that a5 built, not from the global arrays -, rebuilds the cell table of that
 // local set from the particles' positions, and runs the production interaction kernel on it for the
 // cell planes the slab owns.  The rates land in the slab's own range of acc4.  Looping over all slabs
-// must reproduce the global sph_interact result value for value (tests/test_gpu_slabs.py): that is the
-// device-side proof that a halo of width 2h (one cell plane) is sufficient.
+// must reproduce the global sph_interact result (tests/test_gpu_slabs.py) - value for value when every
+// tile at a slab plane fits one candidate batch, to rounding otherwise (interact_mma.cu, DRAIN) -: that
+// is the device-side proof that a halo of width 2h (one cell plane) is sufficient.
 //
 // Local storage: the idle halves of the double-buffered state (dead between the gather and the next
 // sort) and one extra cell table.  With x-major keys the local set is a contiguous piece of the global

@@ -334,6 +334,12 @@ int sph_init(sph_ctx **out, const sph_params *p, const sph_particles *part, int 
     // kernel attributes are per device: set them for the device this context lives on
     cudaError_t e = configure_interact();
     if (e == cudaSuccess) e = configure_sort();
+    int dev = 0;
+    c->num_sms = NUM_SMS;
+    if (e == cudaSuccess) e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e == cudaSuccess && c->num_sms < 1) c->num_sms = NUM_SMS;
+    if (e == cudaSuccess) e = configure_keys(c);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->acc4, 0, 16 * (c->n ? c->n : 1), c->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->mig_total, 0, 4, c->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->mig_count, 0, 4 * 2 * SPH_MAX_SLABS, c->stream);
@@ -511,7 +517,7 @@ int sph_time_step(sph_ctx *c, float cfl, float *dt, float *amax_slab, float *sma
     if (!c->sorted_valid || !c->rates_valid || !c->mu_valid) return SPH_ERR_ORDER;
     uint32_t h[2 * SPH_MAX_SLABS];
     {
-        Timed t(c, SPH_T_VERLET);
+        Timed t(c, SPH_T_DTREDUCE);
         CK(c, launch_dt_reduce(c));
     }
     CK(c, cudaMemcpyAsync(h, c->dt_red, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
@@ -580,6 +586,7 @@ int sph_get_view(sph_ctx *c, sph_view *v)
     v->mig_total = c->mig_total;
     v->migrants = (const uint32_t *)c->migrants;
     v->mig_count = c->mig_count;
+    v->mumax = c->mumax;
     return SPH_OK;
 }
 
@@ -723,10 +730,13 @@ int sph_fma_peak(sph_ctx *c, int variant, int iters, double *tflops)
 {
     if (!c || !tflops || iters < 1 || (variant != 0 && variant != 1)) return SPH_ERR_ARG;
     if (c->sticky) return c->sticky;
-    const int blocks = NUM_SMS * 8;
+    const int blocks = c->num_sms * 8;
     cudaEvent_t e0, e1;
     CK(c, cudaEventCreate(&e0));
-    CK(c, cudaEventCreate(&e1));
+    {
+        cudaError_t ec = cudaEventCreate(&e1);
+        if (ec != cudaSuccess) { cudaEventDestroy(e0); return cuda_fail(c, ec); }
+    }
     float *sink = (float *)c->scratch64;
     int rc = SPH_OK;
     cudaError_t e = launch_fma_peak(c, variant, iters / 8 + 1, blocks, sink);      // warm-up

@@ -11,7 +11,7 @@ constexpr uint32_t CELL_MASK = 0x0FFFFFFFu;   // keyword bits 0..27 = cell label
 constexpr int TAG_SHIFT = 28;                 // bits 28..29 edge label, 30..31 migration label
 constexpr uint32_t ID_MASK = 0x0FFFFFFFu;     // idt bits 0..27 = id, bit 31 = type
 constexpr uint32_t TYPE_BIT = 0x80000000u;
-constexpr int NUM_SMS = 148;                  // B200
+constexpr int NUM_SMS = 148;                  // B200 (fallback; sph_ctx::num_sms is the device's own count)
 constexpr int GATHER_THREADS = 256;           // slots per tile of gather_kernel = tile of the migrant counts
 constexpr int MG_SUB = 16;                    // tiles per group = per CTA of the migrant compaction
 
@@ -79,6 +79,8 @@ struct sph_ctx {
     uint64_t n;
     int max_slabs;
     int cell_bits, passes;
+    int num_sms;               // multiProcessorCount of the context's device (read once in sph_init)
+    int keys_blocks_per_sm;    // resident CTAs per SM of this context's keys_kernel<passes> (one wave per launch)
     cudaStream_t stream;
     int sticky;                // SPH_OK or SPH_ERR_CUDA
 
@@ -95,7 +97,8 @@ struct sph_ctx {
     uint32_t *keyword;         // sorted keywords
     uint32_t *hist;            // passes*256 digit histograms
     uint32_t *tile_state;      // passes * rs_tiles * 256 look-back words
-    uint32_t *counters;        // 64 words: dynamic tile counters [0..3], gap work-list counter [8]
+    uint32_t *counters;        // 64 words: dynamic tile counters of the sort passes [0..3], gap work-list
+                               // counter [8], interaction kernel: tiles listed [16], next tile to hand out [17]
     uint32_t rs_tiles;
     // cells / slabs
     uint32_t *cell_begin;      // ncells+1
@@ -171,6 +174,7 @@ int interact_mma_targets();
 size_t interact_mma_tile_capacity(const int nc[3], int zb);
 int interact_mma_zmax();
 cudaError_t configure_sort();
+cudaError_t configure_keys(sph_ctx *c);        // fills keys_blocks_per_sm (needs c->passes)
 
 uint32_t radix_tiles(uint64_t n);
 uint32_t gather_tiles(uint64_t n);

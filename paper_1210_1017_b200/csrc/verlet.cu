@@ -192,7 +192,7 @@ cudaError_t launch_dt_reduce(sph_ctx *c)
     cudaError_t e = cudaMemsetAsync(c->dt_red, 0, sizeof(uint32_t) * 2 * SPH_MAX_SLABS, c->stream);
     if (e != cudaSuccess || n == 0) return e;
     uint32_t blocks = (n + 255) / 256;
-    if (blocks > (uint32_t)NUM_SMS * 8) blocks = NUM_SMS * 8;
+    if (blocks > (uint32_t)c->num_sms * 8) blocks = (uint32_t)c->num_sms * 8;
     dt_reduce_kernel<<<blocks, 256, 0, c->stream>>>(n, c->acc4, c->velrho4[c->cur], c->mumax, c->idt[c->cur],
                                                    c->slab_begin, c->tagged_slabs.n_slabs, c->phys, c->dt_red);
     c->n_launches++;

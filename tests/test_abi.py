@@ -34,10 +34,10 @@ def test_library_exports_every_declared_symbol(B):
 
 
 def test_struct_layouts_match_header(B):
-    # sizes implied by the header on LP64: params 18 words; particles 7 words of 8; view 6+15*8
+    # sizes implied by the header on LP64: params 19 words; particles 7 words of 8; view 40 B + 16 pointers
     assert C.sizeof(B.sph_params) == 4 * 19
     assert C.sizeof(B.sph_particles) == 8 * 7
-    assert C.sizeof(B.sph_view) == 8 + 12 + 4 + 4 + 4 + 8 + 15 * 8
+    assert C.sizeof(B.sph_view) == 8 + 12 + 4 + 4 + 4 + 8 + 16 * 8
 
 
 def test_workspace_bytes_and_argument_errors(B):

@@ -123,11 +123,13 @@ def test_dense_cells_use_several_batches_and_chunks():
     assert e_d <= TOL_RATE and e_a <= TOL_RATE
 
 
-def test_particles_outside_the_grid_widen_the_fp16_filter():
-    """Reading A13: particles beyond the grid sit clamped in edge cells.  The interaction kernel's
-    fp16 filter is derived for particles inside their cells; a CTA that meets one outside that
-    model must let every candidate through to the exact fp32 evaluation.  Here the grid stops at a
-    third of the tank in x, so the far wall and part of the floor are up to ~17 h outside."""
+def test_particles_outside_the_grid_switch_the_filter_to_wide():
+    """Reading A13: particles beyond the grid sit clamped in edge cells.  The production kernel's tf32
+    distance filter (interact_mma.cu, filter_thr) is derived for records inside the staged region of their
+    tile (|x|, |y| <= 4h, |z| <= (zb + 2) h from the tile centre); a tile that meets a record outside that
+    model sets its "wide" switch (ImStage::wide), which lets every candidate through to the exact fp32 pair
+    term.  Here the grid stops at a third of the tank in x, so the far wall and part of the floor are up to
+    ~17 h outside: the limit reached is the wide switch of the production kernel."""
     w = W.dam_break(12, scrambled=True)
     P = dict(w.params)
     P["dom_max"] = (W.f32(P["dom_min"][0] + 10.0 * 2.0 * P["h"]), P["dom_max"][1], P["dom_max"][2])
@@ -140,8 +142,9 @@ def test_particles_outside_the_grid_widen_the_fp16_filter():
 
 
 def test_sparse_cells_long_z_blocks():
-    """h = 0.75 dp: 3.4 particles per cell, so a CTA owns the maximum run of 32 cells and the fp16
-    filter works with its widest z range (|z| < 64 h) and largest error pad."""
+    """h = 0.75 dp: 3.4 particles per cell, so a tile of the production kernel takes its longest z-block
+    (zb = IM_ZMAX = 6 cells: the tf32 error model at its widest, |z| <= 8 h, and its largest threshold pad);
+    variant 1, the plain 27-cell walk, is the second opinion."""
     w = W.dam_break(16, scrambled=True)
     P = dict(w.params)
     P["h"] = W.f32(0.75 * P["dp"])

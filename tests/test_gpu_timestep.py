@@ -64,6 +64,43 @@ def test_time_step_matches_oracle_bracket(variant, n_slabs, nb):
     assert lo["smax_slab"].max() > 1.02 * c_max
 
 
+@pytest.mark.parametrize("variant", [0, 1])
+def test_mumax_per_particle_on_a_disordered_state(variant):
+    """The filter of the production kernel must never drop a pair with r < 2h (reading A19): a
+    lost pair just inside the cut-off changes a rate by ~1e-6 of a term - invisible at 1e-4 - but it can be
+    the pair that sets max_j |mu_ij| (L112, L150), which does not vanish at r = 2h.  So mumax is compared
+    PARTICLE BY PARTICLE with the oracle's bracket: at least the maximum over the pairs clearly inside
+    (cut = 1 - 1e-5), at most the one over the pairs up to just outside (cut = 1 + 1e-5)."""
+    w = W.dam_break(32, scrambled=True)
+    nf = w.n_fluid
+    ids = np.arange(nf, dtype=np.int64)
+    pos = w.pos.astype(np.float64)
+    for c in range(3):
+        pos[:nf, c] += (2.0 * W.u01(W.SEED_STATE + 7, ids, c) - 1.0) * 0.3 * w.params["dp"]
+    w.pos = pos.astype(np.float32)
+    sph = make_sph(w)
+    sph.sph_set_option(B.SPH_OPT_INTERACT_VARIANT, variant)
+    sph.sph_set_option(B.SPH_OPT_ADAPTIVE_DT, 1)
+    sph.sph_sort_and_cells()
+    sph.sph_interact()
+    T = sph.view_tensors()
+    assert sph.sph_status() == 0
+    order = T["idt"].cpu().numpy().view(np.uint32) & 0x0FFFFFFF
+    mu = np.empty(w.n, dtype=np.float64)
+    mu[order] = T["mumax"].cpu().numpy()
+    p = OB.params_from_workload(w.params)
+    acc, _ = OB.rates(p, w.pos, w.vel, w.rho, w.type)
+    lo = OB.time_step(p, w.pos, w.vel, w.rho, w.type, acc, CFL, cut=1.0 - EPS)["mu"]
+    hi = OB.time_step(p, w.pos, w.vel, w.rho, w.type, acc, CFL, cut=1.0 + EPS)["mu"]
+    scale = hi.max()
+    assert scale > 0 and (lo > 0).mean() > 0.5
+    tol = 2e-5 * scale                               # fp32 evaluation of h v.r / (r^2 + eta^2)
+    worst_lo, worst_hi = (lo - mu).max() / scale, (mu - hi).max() / scale
+    print(f"mumax per particle, variant {variant}: below lower bracket by {worst_lo:.2e}, above upper by {worst_hi:.2e} (of max mu)")
+    assert np.all(mu >= lo - tol), "a pair inside the cut-off was lost"
+    assert np.all(mu <= hi + tol), "a pair outside the cut-off was counted"
+
+
 def test_time_step_needs_mu():
     w = W.dam_break(8, scrambled=True)
     sph = make_sph(w)
