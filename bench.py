@@ -38,7 +38,7 @@ FLOPS_PER_CANDIDATE, FLOPS_PER_PAIR = 8, 32      # DESIGN.md "interaction flop c
 # an `ncu --set full` capture of this command (DRAM counters cannot be read inside a timed run): config ->
 # (bytes, file under profiles/ that holds the capture).  Configs without a capture report null.
 IA_TRAFFIC = {3: (3316548096 + 533717760, "ncu capture profiles/r02_opmix_config3.md (dram__bytes_read.sum + dram__bytes_write.sum)")}
-IA_KERNEL = {0: "interact_mma_kernel", 1: "interact_simple_kernel", 2: "interact_staged_kernel"}
+IA_KERNEL = {0: "interact_mma_kernel", 1: "interact_simple_kernel"}
 # algorithmic HBM bytes per particle of the memory-bound stages
 # dt_reduce (sph_time_step): acc4 16 + velrho4 16 + mumax 4 + idt 4 B read per particle
 BYTES = dict(keys=28.0, sort_per_pass=16.0, gather=116.0, verlet=116.0, migrate=4.0, dt_reduce=40.0)
@@ -294,6 +294,8 @@ def main():
                     help="after the main measurement (config 3, N = 1 only), run the sort/halo microbenchmark at 2^LOG2N "
                          "in the same process and attach it to the JSON line under 'micro' (0 = skip)")
     ap.add_argument("--variant", type=int, default=0)
+    ap.add_argument("--kernel", type=int, default=0, choices=[0, 1],
+                    help="smoothing kernel: 0 = Wendland C2 (BASELINE configs), 1 = cubic spline (the paper's own, L81)")
     ap.add_argument("--disorder", type=int, default=0, metavar="K",
                     help="time a DISORDERED fluid instead of the rest-state lattice: scrambled start (random "
                          "velocities 0.1 sqrt(gH), densities rho0 (1 + U(0, 1 %%))) stepped K times before warm-up")
@@ -324,6 +326,9 @@ def main():
 
     nb = CONFIG_NB[args.config]
     w = W.dam_break(nb, scrambled=args.disorder > 0)
+    if args.kernel:
+        w.params = dict(w.params)
+        w.params["kernel"] = args.kernel
     sph = B.Sph(w.params, w.pos, w.vel, w.rho, w.type, device=f"cuda:{local}")
     sph.sph_set_option(B.SPH_OPT_INTERACT_VARIANT, args.variant)
     v = sph.sph_get_view()
@@ -450,7 +455,7 @@ def main():
     sm_mhz = clocks.get("sm_mhz") or pk["sm_max_mhz"]
     # the FP32 peak this box really sustains: register-resident FMA chains, same process (csrc/fma_peak.cu)
     peak_meas = max(sph.sph_fma_peak(0, 8192), sph.sph_fma_peak(1, 8192))
-    traffic, traffic_src = IA_TRAFFIC.get(args.config if not (args.disorder or args.adaptive or args.variant) else None, (None, None))
+    traffic, traffic_src = IA_TRAFFIC.get(args.config if not (args.disorder or args.adaptive or args.variant or args.kernel) else None, (None, None))
     roofline = dict(bound="alu", kernel=IA_KERNEL.get(args.variant, "?"), achieved=achieved, peak=peak, unit="TFLOP/s",
                     frac=achieved / peak, traffic=traffic, traffic_source=traffic_src,
                     peak_source=f"148 SMs x 128 FP32 lanes x 2 flop x {pk['sm_max_mhz']:.0f} MHz (max clock, {pk['source']})",
@@ -482,7 +487,7 @@ def main():
     # ---- BASELINE.json configs[4] on the same line: the >= 60 % HBM bars of the sort and compaction kernels
     # are quoted on the random-order microbenchmark, not on the (nearly sorted) simulation state
     micro = None
-    if args.main_micro and world == 1 and args.config == 3 and not (args.adaptive or args.disorder or args.variant):
+    if args.main_micro and world == 1 and args.config == 3 and not (args.adaptive or args.disorder or args.variant or args.kernel):
         sph.sph_destroy()
         del sph, T, pin, outp
         torch.cuda.empty_cache()
@@ -506,6 +511,7 @@ def main():
                              f"particles, {w.n_slabs} logical x-slabs",
                     state=(f"disordered: scrambled start + {args.disorder} steps before warm-up" if args.disorder
                            else "rest-state lattice with seeded jitter (BASELINE configs)"),
+                    smoothing_kernel=("cubic spline (PAPER.md L81)" if args.kernel else "Wendland C2 (BASELINE.json)"),
                     n_particles=n, n_slabs=w.n_slabs, cells=int(v.ncells), cell_bits=int(v.cell_bits),
                     radix_passes=passes, dt=("variable, cfl 0.2" if args.adaptive else w.dt), multi_gpu="replicas only",
                     l2="no flush: per-step working set %.1f GB >> 126 MB L2" % (n * 198e-9)

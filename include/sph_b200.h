@@ -123,8 +123,7 @@ enum {
 /* Options for sph_set_option. */
 enum {
     SPH_OPT_INTERACT_VARIANT = 0, /* 0 = production kernel, 1 = simple one-thread-per-particle
-                                     kernel (cross-check), 2 = the round-1 staged kernel with the
-                                     fp16 ALU filter (cross-check) */
+                                     kernel (cross-check); other values: SPH_ERR_ARG */
     SPH_OPT_ADAPTIVE_DT = 1       /* 1 = sph_interact also records max_j |mu_ij| of every particle,
                                      which sph_time_step needs (costs a few instructions per pair);
                                      0 (default) = fixed-dt path */

@@ -319,12 +319,6 @@ int sph_init(sph_ctx **out, const sph_params *p, const sph_particles *part, int 
     c->prev_init = (uint8_t *)(w + L.prev_init);
     c->flags = (uint32_t *)(w + L.flags);
     c->interact_variant = 0;
-    // cells per z-block of the interaction kernel: fill the CTA's threads with targets
-    double ppc = pow(2.0 * (double)p->h / (double)p->dp, 3.0);
-    int zb = (int)floor((double)interact_threads() * 0.97 / (ppc > 0.05 ? ppc : 0.05));
-    if (zb < 1) zb = 1;
-    if (zb > 32) zb = 32;
-    c->zblock = zb;
     c->zblock_mma = mma_zblock(p);
     c->ia_tiles = (uint32_t *)(w + L.ia_tiles);
 
@@ -628,7 +622,7 @@ int sph_set_option(sph_ctx *c, int option, int value)
     if (!c) return SPH_ERR_ARG;
     switch (option) {
     case SPH_OPT_INTERACT_VARIANT:
-        if (value < 0 || value > 2) return SPH_ERR_ARG;
+        if (value < 0 || value > 1) return SPH_ERR_ARG;
         c->interact_variant = value;
         return SPH_OK;
     case SPH_OPT_ADAPTIVE_DT:

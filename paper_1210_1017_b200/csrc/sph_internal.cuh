@@ -127,7 +127,6 @@ struct sph_ctx {
     int adaptive_dt;           // SPH_OPT_ADAPTIVE_DT: sph_interact also produces mumax
     uint64_t step_index;
     int interact_variant;
-    int zblock;                // cells per z-block of the staged (round-1) interaction kernel
     int zblock_mma;            // cells per z-block of a tile of the production interaction kernel
 
     uint64_t n_launches;       // kernels launched so far (memsets and copies not counted)
@@ -180,7 +179,6 @@ uint32_t radix_tiles(uint64_t n);
 uint32_t gather_tiles(uint64_t n);
 uint32_t mig_groups(uint64_t n);
 size_t gap_list_entries(uint64_t ncells);
-int interact_threads();
 
 // Tait pressure over rho^2 from rho, fp32, cancellation-free.
 __device__ __forceinline__ float tait_p_over_rho2(float rho, const PhysC &ph)

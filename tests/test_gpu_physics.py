@@ -31,7 +31,7 @@ def _gpu_rates(w, variant=0, planes=None):
     return out
 
 
-@pytest.mark.parametrize("variant", [0, 1, 2])
+@pytest.mark.parametrize("variant", [0, 1])
 def test_config0_rest_state_rates(variant):
     """Prescribed check: config 0 at rest.  p = 0 and v = 0, so every fluid rate is (g, 0)."""
     w = W.dam_break(16)
@@ -44,7 +44,7 @@ def test_config0_rest_state_rates(variant):
     assert np.array_equal(out["pos"], w.pos) and np.array_equal(out["rho"], w.rho)
 
 
-@pytest.mark.parametrize("variant", [0, 1, 2])
+@pytest.mark.parametrize("variant", [0, 1])
 def test_disordered_positions_rates(variant):
     """No lattice: every fluid particle is moved by U(-0.3, 0.3) dp per axis (seeded), on top of random
     velocities and densities.  Neighbour counts then differ from particle to particle (the lanes of a warp
@@ -65,7 +65,7 @@ def test_disordered_positions_rates(variant):
     assert e_a <= TOL_RATE, e_a
 
 
-@pytest.mark.parametrize("variant", [0, 1, 2])
+@pytest.mark.parametrize("variant", [0, 1])
 @pytest.mark.parametrize("nb", [16, 40])
 def test_scrambled_state_rates(variant, nb):
     """Reading A21: same positions, random velocities and densities, so that pressure,
@@ -91,7 +91,7 @@ def test_variants_agree_and_slabs_do_not_change_rates():
     assert np.array_equal(a["acc"], c["acc"]) and np.array_equal(a["drho"], c["drho"])
 
 
-@pytest.mark.parametrize("variant", [0, 1, 2])
+@pytest.mark.parametrize("variant", [0, 1])
 def test_nonuniform_mass_and_cubic_spline(variant):
     w = W.dam_break(12, scrambled=True)
     w.params = dict(w.params)
@@ -205,11 +205,15 @@ def test_scrambled_ten_steps_with_corrective_period_and_slabs():
     assert rel_l2(out["drho"], s.drho) <= 5e-3
 
 
-def test_config1_full_size_sampled_rates():
+@pytest.mark.parametrize("kernel", [0, 1])
+def test_config1_full_size_sampled_rates(kernel):
     """BASELINE config 1 (1.2 M particles) at full size, scrambled state, in the launch
     configuration bench.py uses; the oracle evaluates a sample of particles one neighbourhood
-    at a time (all particles within 2h of the sample, brute force)."""
+    at a time (all particles within 2h of the sample, brute force).  kernel = 1: the cubic spline the
+    paper itself used (L81; NEXT-2 of SURVEY 8(f)) at the same size."""
     w = W.dam_break(100, scrambled=True)
+    w.params = dict(w.params)
+    w.params["kernel"] = kernel
     out = _gpu_rates(w, 0)
     p = OB.params_from_workload(w.params)
     rng_ids = (W.u01(77, np.arange(64), 0) * w.n).astype(np.int64)

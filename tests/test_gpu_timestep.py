@@ -36,7 +36,7 @@ def test_some_case_has_a_ragged_last_warp():
     assert any(W.dam_break(nb).n % 32 != 0 for nb in (16, 13))
 
 
-@pytest.mark.parametrize("variant", [0, 1, 2])
+@pytest.mark.parametrize("variant", [0, 1])
 @pytest.mark.parametrize("n_slabs,nb", [(1, 16), (3, 16), (3, 13)])
 def test_time_step_matches_oracle_bracket(variant, n_slabs, nb):
     w = W.dam_break(nb, scrambled=True, n_slabs=n_slabs)
