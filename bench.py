@@ -37,7 +37,8 @@ FLOPS_PER_CANDIDATE, FLOPS_PER_PAIR = 8, 32      # DESIGN.md "interaction flop c
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the production interaction kernel, from
 # an `ncu --set full` capture of this command (DRAM counters cannot be read inside a timed run): config ->
 # (bytes, file under profiles/ that holds the capture).  Configs without a capture report null.
-IA_TRAFFIC = {3: (3316548096 + 533717760, "ncu capture profiles/r02_opmix_config3.md (dram__bytes_read.sum + dram__bytes_write.sum)")}
+IA_TRAFFIC = {3: (3284194000 + 532750848, "ncu capture profiles/r03_ncu_full_config3.md (dram__bytes_read.sum + dram__bytes_write.sum), "
+                  "final build of round 3")}
 IA_KERNEL = {0: "interact_mma_kernel", 1: "interact_simple_kernel"}
 # algorithmic HBM bytes per particle of the memory-bound stages
 # dt_reduce (sph_time_step): acc4 16 + velrho4 16 + mumax 4 + idt 4 B read per particle

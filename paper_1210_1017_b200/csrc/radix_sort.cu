@@ -35,6 +35,26 @@ constexpr uint32_t LB_AGG = 1u << 30;             // look-back word: flag in bit
 constexpr uint32_t LB_INC = 2u << 30;
 constexpr uint32_t LB_VAL = (1u << 30) - 1u;
 
+// Phase clocks of a tile (thread 0 of every CTA), summed over tiles: only in builds with -DSPH_RS_PROFILE
+// (a measurement harness that includes this file and reads rs_prof); the product library is built without
+// it.  Round-3 figures at 2^26 random keys, cycles per tile as thread 0 sees them: load 1900, rank 7200,
+// counts + publish + scans 2400, reorder 4000, look-back 5200 + 900, scatter 3100.
+#ifdef SPH_RS_PROFILE
+__device__ unsigned long long rs_prof[8];
+#define RS_MARK(k)                                                                     \
+    do {                                                                               \
+        if (threadIdx.x == 0) {                                                        \
+            const long long now__ = clock64();                                         \
+            atomicAdd(&rs_prof[k], (unsigned long long)(now__ - rs_t__));              \
+            rs_t__ = now__;                                                            \
+        }                                                                              \
+    } while (0)
+#define RS_MARK_INIT long long rs_t__ = clock64()
+#else
+#define RS_MARK(k) do { } while (0)
+#define RS_MARK_INIT do { } while (0)
+#endif
+
 uint32_t radix_tiles(uint64_t n) { return (uint32_t)((n + RS_TILE - 1) / RS_TILE); }
 
 __device__ __forceinline__ uint32_t ld_relaxed(const uint32_t *p)
@@ -91,6 +111,11 @@ __device__ __forceinline__ void onesweep_tile(RsSmem &S, uint32_t n, const uint2
     const uint32_t bit16 = 1u << lane16, lt16 = bit16 - 1u;
     const uint32_t base = tile * RS_TILE;
     const uint32_t tile_n = FULL ? (uint32_t)RS_TILE : n - base;
+    RS_MARK_INIT;
+    const uint32_t hcount_pre = hist[tid & 255u];       // whole-array count of this thread's digit: needed only
+                                                        // after the ranking, fetched now so that nobody waits for it
+                                                        // between two barriers (1200 cycles per tile in the
+                                                        // instrumented harness; no gain in the product build)
 
     // ---- load, striped per half-warp: the unit owns a contiguous chunk; item k of its lane l is
     // chunk[k*16+l], so that (unit, row, lane) order is index order.
@@ -104,6 +129,10 @@ __device__ __forceinline__ void onesweep_tile(RsSmem &S, uint32_t n, const uint2
         const uint32_t li = ubase + k * 16 + lane16;
         kv[k] = (FULL || li < tile_n) ? __ldcs(in + base + li) : make_uint2(0xFFFFFFFFu, 0u);
     }
+#ifdef SPH_RS_PROFILE
+    if (kv[RS_IPT - 1].x == 0x12345678u && kv[0].y == 0x9ABCDEF0u) rs_prof[7] = 1;      // wait for the loads
+#endif
+    RS_MARK(0);                                                                          // load
     // ---- rank inside the warp, stable in item order; two 16-bit ranks per register
     uint32_t rank2[RS_IPT / 2];
     const uint32_t tab_addr = (uint32_t)__cvta_generic_to_shared(S.hw[unit]);
@@ -115,6 +144,7 @@ __device__ __forceinline__ void onesweep_tile(RsSmem &S, uint32_t n, const uint2
         if (k & 1) rank2[k >> 1] |= r << 16; else rank2[k >> 1] = r;
     }
     __syncthreads();
+    RS_MARK(1);                                                                          // rank
 
     // ---- per digit (threads 0..255): counts over warps, publish the tile aggregate at once, and
     // put the first round of look-back polls in flight; their latency (and the predecessors'
@@ -137,7 +167,7 @@ __device__ __forceinline__ void onesweep_tile(RsSmem &S, uint32_t n, const uint2
             poll[b] = ((int)tile - 1 - b >= 0) ? ld_relaxed(st - (size_t)(b + 1) * 256) : LB_INC;
 
         uint32_t inc = count;                                       // tile counts over digits
-        uint32_t hcount = hist[tid], hinc = hcount;                 // whole-array counts over digits
+        uint32_t hcount = hcount_pre, hinc = hcount;                // whole-array counts over digits
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
             uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
@@ -164,6 +194,7 @@ __device__ __forceinline__ void onesweep_tile(RsSmem &S, uint32_t n, const uint2
         for (int u = 0; u < RS_UNITS; ++u) S.hw[u][tid] += dstart;
     }
     __syncthreads();
+    RS_MARK(2);                                                                          // counts, publish, scans
 
     // ---- reorder the tile through shared memory (needs only tile-local offsets)
 #pragma unroll
@@ -173,7 +204,10 @@ __device__ __forceinline__ void onesweep_tile(RsSmem &S, uint32_t n, const uint2
         S.stage[tab[d] + r] = kv[k];
     }
 
-    // ---- finish the look-back: same digit in earlier tiles, RS_LB polls per round
+    RS_MARK(3);                                                                          // reorder (thread 0's share)
+    // ---- finish the look-back: same digit in earlier tiles, RS_LB polls per round.  (Rounds of 16, 32 or 64
+    // polls were measured in round 3 and are slower, 2746 / 2673 / 2464 against 2810 GB/s: the wait is for
+    // predecessors that have not published yet, not for the number of words to add up.)
     if (tid < 256) {
         uint32_t lookback = 0;
         if (tile > 0) {
@@ -200,7 +234,9 @@ __device__ __forceinline__ void onesweep_tile(RsSmem &S, uint32_t n, const uint2
         }
         S.gbase[tid] += lookback;
     }
+    RS_MARK(4);                                                                          // look-back of digit 0
     __syncthreads();
+    RS_MARK(5);                                                                          // ... of the slowest digit, reorder of the slowest warp
     // ---- runs of equal digits go to consecutive global addresses
 #pragma unroll
     for (int k = 0; k < RS_IPT; ++k) {
@@ -211,6 +247,7 @@ __device__ __forceinline__ void onesweep_tile(RsSmem &S, uint32_t n, const uint2
             out[S.gbase[d] + i] = e;
         }
     }
+    RS_MARK(6);                                                                          // scatter (issue)
 }
 
 __global__ void __launch_bounds__(RS_THREADS, SPH_RS_MINBLOCKS)
